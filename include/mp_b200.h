@@ -1,0 +1,132 @@
+/* mp_b200.h -- C ABI of the B200-native Matching Pursuit library (libmp_b200.so).
+ *
+ * The method is the Matching Pursuit (MP) iteration of arxiv 0809.1833 (M. Andrecut), cited below as
+ * "P:n" = line n of PAPER.md:
+ *
+ *     t <- 0, x~ <- 0, r <- y                                        Eq. 8,
+ *     while ||r||_2 > eps ||y||_2 and t < T:
+ *         i  <- argmax_m |<r, psi_m>|   (smallest index on ties)      Eq. 9,  P:73;  Eq. 16
+ *         x~_i <- x~_i + <r, psi_i>                                   Eq. 10
+ *         r  <- r - <r, psi_i> psi_i                                  Eq. 11
+ *         t  <- t + 1                                                 Eq. 12
+ *     return x~ (and r, t)
+ *
+ * over a dictionary Psi (N x M) whose columns psi_m have unit l2 norm (Eq. 4).
+ *
+ * CONVENTIONS (all entry points unless stated otherwise)
+ *   - Every data pointer is a DEVICE pointer on the current CUDA device, caller-owned, 16-byte
+ *     aligned, fp32 (int32 for indices / counters).  The *_host entry points at the end take HOST
+ *     pointers instead and say so.
+ *   - The dictionary is ATOM-MAJOR: psi_t[m*ld + n] = Psi[n][m], m = 0..M-1 (atom / column of Psi),
+ *     n = 0..N-1, ld >= N and ld % 4 == 0.  (= Psi^T row-major = Psi column-major; each atom is
+ *     contiguous so the reduction over n is coalesced.)  Elements psi_t[m*ld + n], N <= n < ld, may
+ *     be read by the library but never influence a result.  The paper's own layout (Psi row-major,
+ *     A2 P:360) is NOT accepted.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Calls are
+ *     asynchronous on `stream`: they validate arguments on the host, enqueue work and return; they
+ *     never synchronise the host (exception: the stream-loop fallback algorithm, see mp_set_int).
+ *     All outputs, n_iter included, are device memory and valid once the stream has reached the
+ *     end of the call.
+ *   - The library allocates nothing on the hot path and keeps no per-problem state between calls;
+ *     the caller provides `workspace` (>= mp_workspace_bytes(N, M, B) bytes, 256-byte aligned).
+ *   - Errors: a status code is returned, nothing is printed, nothing throws.  Argument errors are
+ *     detected before anything is enqueued and leave every output untouched.  mp_last_error()
+ *     describes the most recent failure on the calling thread.
+ *   - Indices are 0-based.  Non-finite inputs: results unspecified, but the call
+ *     terminates within max_iter iterations and a NaN correlation never wins the argmax.
+ */
+#ifndef MP_B200_H
+#define MP_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#if defined(__GNUC__)
+#define MP_API __attribute__((visibility("default")))
+#else
+#define MP_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    MP_OK = 0,
+    MP_ERR_INVALID_ARG = 1, /* null / misaligned pointer, N<1, M<1, B<1, max_iter<0, eps<0 or NaN, ld<N, ld%4 */
+    MP_ERR_CUDA = 2,        /* a CUDA runtime call or launch failed; see mp_last_error() */
+    MP_ERR_UNSUPPORTED = 3, /* shape outside what the selected algorithm supports */
+    MP_ERR_WORKSPACE = 4    /* workspace null, misaligned or smaller than mp_workspace_bytes() */
+} mp_status;
+
+/* Bytes of device workspace mp_recover (B = 1) / mp_recover_batched (B signals) need.  0 on invalid sizes. */
+MP_API size_t mp_workspace_bytes(int N, int M, int B);
+
+/* Column normalisation, Eq. 4: psi_m <- psi_m / ||psi_m||_2 for every atom, in place.
+ * The sum of squares is accumulated in float64 and each element is divided in float64 and rounded to
+ * fp32 once.  A zero atom is left zero.  norms_out (M floats, nullable) receives the norms BEFORE
+ * scaling.  The paper assumes Eq. 4 and never executes it (its Bernoulli atoms are unit by
+ * construction, Eq. 13). */
+MP_API mp_status mp_normalize_columns(float* psi_t, int N, int M, int64_t ld, float* norms_out, void* stream);
+
+/* The MP loop above for one signal.
+ *   psi_t      in   dictionary, ASSUMED column-normalised (not checked; the update uses <r,psi_i> as is)
+ *   y          in   N measurements, y = Psi x (Eq. 2)
+ *   eps        in   stop once ||r||_2 <= eps*||y||_2 (tested at the top of the loop)
+ *   max_iter   in   T of Eq. 8 / P:88;  max_iter = 0 or y = 0 returns x~ = 0, r = y, n_iter = 0
+ *   x          out  M floats, x~ (zeroed by the call, then accumulated in float64, rounded once at the end)
+ *   r          out  N floats, the final residual (held in float64 inside the call, rounded once)
+ *   n_iter     out  1 int, number of completed updates t
+ *   idx_trace  out  nullable, max_iter ints:   atom chosen at iteration t, for t < n_iter
+ *   c_trace    out  nullable, max_iter floats: the signed <r,psi_i> added at iteration t
+ * Arithmetic: correlations are fp32 dot products of an fp32 rounding of r; r itself, ||r||^2 (a direct sum of
+ * squares every iteration, as nrm2 at A2 P:471) and the stop test are float64. */
+MP_API mp_status mp_recover(const float* psi_t, int N, int M, int64_t ld,
+                     const float* y, float eps, int max_iter,
+                     float* x, float* r, int* n_iter,
+                     int* idx_trace, float* c_trace,
+                     void* workspace, size_t workspace_bytes, void* stream);
+
+/* B signals sharing one dictionary ("all signals are encoded/decoded with the same dictionary").
+ * Signal b's result equals mp_recover on (psi_t, Y[b]); signals are independent and a signal that has
+ * stopped is frozen (x_b, r_b, n_iter_b no longer change) while the others continue.
+ *   Y  in  B x N row-major, row stride ldy >= N (ldy % 4 == 0);   X out B x M;   R out B x N;   n_iter out B ints.
+ * The correlation step is the dense contraction Psi^T R. */
+MP_API mp_status mp_recover_batched(const float* psi_t, int N, int M, int64_t ld,
+                             const float* Y, int64_t ldy, int B,
+                             float eps, int max_iter,
+                             float* X, float* R, int* n_iter,
+                             void* workspace, size_t workspace_bytes, void* stream);
+
+/* Description of the last error on this thread ("" if none).  Static storage, never NULL. */
+MP_API const char* mp_last_error(void);
+
+/* Tuning / diagnostic knobs (process-wide, not part of the method).  Unknown name -> MP_ERR_INVALID_ARG.
+ *   "algo"          0 = auto (default), 1 = persistent cooperative kernel, 2 = stream loop of small kernels
+ *                   (general fallback; synchronises the host every "chunk" iterations to read the stop flag)
+ *   "warps"         consumer warps per CTA of the persistent kernel (0 = auto)
+ *   "slot_bytes"    bytes of one shared-memory stage (0 = auto);   "depth"  stages per warp (0 = auto)
+ *   "grid"          CTAs of the persistent kernel (0 = auto = one per SM)
+ *   "chunk"         iterations enqueued between stop-flag polls of algo 2 (default 64) */
+MP_API mp_status mp_set_int(const char* name, int64_t value);
+MP_API mp_status mp_get_int(const char* name, int64_t* value);
+
+/* Number of kernels the library has launched on behalf of this process so far (for bench.py's gpu_launches). */
+MP_API int64_t mp_launch_count(void);
+
+/* ---- HOST-buffer entry points (end-to-end convenience; every pointer below is a HOST pointer) ----------
+ * mp_recover_host allocates device buffers, copies psi_t (M*ld floats) and y to the device on an internal
+ * stream, optionally normalises the columns on the device (normalize != 0; the host copy of psi_t is not
+ * modified), runs mp_recover, copies x, r, n_iter (and the traces if non-null) back, synchronises and frees.
+ * Pinned host memory makes the copies faster but is not required.  mp_recover_batched_host likewise. */
+MP_API mp_status mp_recover_host(const float* psi_t, int N, int M, int64_t ld, int normalize,
+                          const float* y, float eps, int max_iter,
+                          float* x, float* r, int* n_iter, int* idx_trace, float* c_trace);
+MP_API mp_status mp_recover_batched_host(const float* psi_t, int N, int M, int64_t ld, int normalize,
+                                  const float* Y, int64_t ldy, int B, float eps, int max_iter,
+                                  float* X, float* R, int* n_iter);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MP_B200_H */

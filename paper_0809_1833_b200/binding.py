@@ -1,0 +1,217 @@
+"""Thin Python binding of libmp_b200.so (include/mp_b200.h).  Argument marshalling only: every step
+of the Matching Pursuit path runs in the library's CUDA kernels.  PyTorch supplies device memory and
+streams.  There is no CPU fallback: a missing library or a failed call raises.
+
+Function names and argument order follow the C header; see include/mp_b200.h for the contract
+(citations into PAPER.md, layouts, ownership, error behaviour).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import dataclasses
+import os
+
+import torch
+
+from . import build as _build
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+class MPError(RuntimeError):
+    def __init__(self, status: int, message: str):
+        super().__init__(f"mp_b200 status {status} ({_STATUS.get(status, '?')}): {message}")
+        self.status = status
+
+
+_STATUS = {0: "MP_OK", 1: "MP_ERR_INVALID_ARG", 2: "MP_ERR_CUDA", 3: "MP_ERR_UNSUPPORTED", 4: "MP_ERR_WORKSPACE"}
+MP_OK, MP_ERR_INVALID_ARG, MP_ERR_CUDA, MP_ERR_UNSUPPORTED, MP_ERR_WORKSPACE = range(5)
+
+
+def _load():
+    path = _build.LIB
+    if not os.path.exists(path):
+        try:
+            _build.build()
+        except Exception as e:  # loud: no fallback implementation exists
+            raise ImportError(f"libmp_b200.so is missing and could not be built with nvcc: {e}") from e
+    return C.CDLL(path)
+
+
+lib = _load()
+_vp, _i, _i64, _f, _sz = C.c_void_p, C.c_int, C.c_int64, C.c_float, C.c_size_t
+lib.mp_workspace_bytes.restype = _sz
+lib.mp_workspace_bytes.argtypes = [_i, _i, _i]
+lib.mp_normalize_columns.restype = _i
+lib.mp_normalize_columns.argtypes = [_vp, _i, _i, _i64, _vp, _vp]
+lib.mp_recover.restype = _i
+lib.mp_recover.argtypes = [_vp, _i, _i, _i64, _vp, _f, _i, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]
+lib.mp_recover_batched.restype = _i
+lib.mp_recover_batched.argtypes = [_vp, _i, _i, _i64, _vp, _i64, _i, _f, _i, _vp, _vp, _vp, _vp, _sz, _vp]
+lib.mp_last_error.restype = C.c_char_p
+lib.mp_last_error.argtypes = []
+lib.mp_set_int.restype = _i
+lib.mp_set_int.argtypes = [C.c_char_p, _i64]
+lib.mp_get_int.restype = _i
+lib.mp_get_int.argtypes = [C.c_char_p, C.POINTER(_i64)]
+lib.mp_launch_count.restype = _i64
+lib.mp_launch_count.argtypes = []
+lib.mp_recover_host.restype = _i
+lib.mp_recover_host.argtypes = [_vp, _i, _i, _i64, _i, _vp, _f, _i, _vp, _vp, _vp, _vp, _vp]
+lib.mp_recover_batched_host.restype = _i
+lib.mp_recover_batched_host.argtypes = [_vp, _i, _i, _i64, _i, _vp, _i64, _i, _f, _i, _vp, _vp, _vp]
+
+
+def _check(status: int):
+    if status != 0:
+        raise MPError(status, lib.mp_last_error().decode())
+
+
+def mp_last_error() -> str:
+    return lib.mp_last_error().decode()
+
+
+def mp_set_int(name: str, value: int) -> None:
+    _check(lib.mp_set_int(name.encode(), int(value)))
+
+
+def mp_get_int(name: str) -> int:
+    v = _i64(0)
+    _check(lib.mp_get_int(name.encode(), C.byref(v)))
+    return v.value
+
+
+def mp_launch_count() -> int:
+    return lib.mp_launch_count()
+
+
+def mp_workspace_bytes(N: int, M: int, B: int = 1) -> int:
+    return lib.mp_workspace_bytes(N, M, B)
+
+
+def _stream_ptr(stream) -> int:
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return stream.cuda_stream
+
+
+def _dict_args(psi_t: torch.Tensor):
+    if not (psi_t.is_cuda and psi_t.dtype == torch.float32 and psi_t.dim() == 2 and (psi_t.shape[1] == 1 or psi_t.stride(1) == 1)):
+        raise TypeError("psi_t must be a CUDA float32 [M, N] tensor with unit stride along N (atom-major)")
+    M, N = psi_t.shape
+    ld = psi_t.stride(0) if M > 1 else max(psi_t.stride(0), N)
+    return psi_t.data_ptr(), N, M, ld
+
+
+def _dev(t: torch.Tensor, dtype, what: str):
+    if not (t.is_cuda and t.dtype == dtype and t.is_contiguous()):
+        raise TypeError(f"{what} must be a contiguous CUDA {dtype} tensor")
+    return t.data_ptr()
+
+
+def _workspace(N, M, B, workspace, device):
+    need = mp_workspace_bytes(N, M, B)
+    if workspace is None:
+        workspace = torch.empty(need + 256, dtype=torch.uint8, device=device)
+    base = workspace.data_ptr()
+    off = (-base) % 256
+    return workspace, base + off, workspace.numel() - off
+
+
+def mp_normalize_columns(psi_t: torch.Tensor, norms_out: torch.Tensor | None = None, stream=None) -> None:
+    """Eq. 4, in place on the device tensor psi_t[M, N]."""
+    p, N, M, ld = _dict_args(psi_t)
+    n = _dev(norms_out, torch.float32, "norms_out") if norms_out is not None else None
+    with torch.cuda.device(psi_t.device):
+        _check(lib.mp_normalize_columns(p, N, M, ld, n, _stream_ptr(stream)))
+
+
+@dataclasses.dataclass
+class Recovered:
+    x: torch.Tensor                      # [M] (or [B, M]) float32, device
+    r: torch.Tensor                      # [N] (or [B, N]) float32, device
+    n_iter: torch.Tensor                 # [1] (or [B]) int32, device
+    idx_trace: torch.Tensor | None = None
+    c_trace: torch.Tensor | None = None
+    workspace: torch.Tensor | None = None
+
+
+def mp_recover(psi_t: torch.Tensor, y: torch.Tensor, eps: float, max_iter: int, *, x=None, r=None, n_iter=None,
+               idx_trace=None, c_trace=None, trace: bool = False, workspace=None, stream=None) -> Recovered:
+    """Eq. 8-12 for one signal; asynchronous on the stream, outputs are device tensors."""
+    p, N, M, ld = _dict_args(psi_t)
+    dev = psi_t.device
+    if y.numel() != N:
+        raise ValueError("y must have N elements")
+    x = torch.empty(M, dtype=torch.float32, device=dev) if x is None else x
+    r = torch.empty(N, dtype=torch.float32, device=dev) if r is None else r
+    n_iter = torch.empty(1, dtype=torch.int32, device=dev) if n_iter is None else n_iter
+    if trace and idx_trace is None:
+        idx_trace = torch.empty(max(max_iter, 1), dtype=torch.int32, device=dev)
+    if trace and c_trace is None:
+        c_trace = torch.empty(max(max_iter, 1), dtype=torch.float32, device=dev)
+    workspace, wp, wb = _workspace(N, M, 1, workspace, dev)
+    with torch.cuda.device(dev):
+        _check(lib.mp_recover(p, N, M, ld, _dev(y, torch.float32, "y"), float(eps), int(max_iter),
+                              _dev(x, torch.float32, "x"), _dev(r, torch.float32, "r"), _dev(n_iter, torch.int32, "n_iter"),
+                              _dev(idx_trace, torch.int32, "idx_trace") if idx_trace is not None else None,
+                              _dev(c_trace, torch.float32, "c_trace") if c_trace is not None else None,
+                              wp, wb, _stream_ptr(stream)))
+    return Recovered(x, r, n_iter, idx_trace, c_trace, workspace)
+
+
+def mp_recover_batched(psi_t: torch.Tensor, Y: torch.Tensor, eps: float, max_iter: int, *, X=None, R=None, n_iter=None,
+                       workspace=None, stream=None) -> Recovered:
+    """B signals sharing psi_t: Y[B, N] -> X[B, M], R[B, N], n_iter[B]."""
+    p, N, M, ld = _dict_args(psi_t)
+    dev = psi_t.device
+    if not (Y.is_cuda and Y.dtype == torch.float32 and Y.dim() == 2 and Y.shape[1] == N and Y.stride(1) == 1):
+        raise TypeError("Y must be a CUDA float32 [B, N] tensor with unit stride along N")
+    B = Y.shape[0]
+    ldy = Y.stride(0) if B > 1 else max(Y.stride(0), N)
+    X = torch.empty(B, M, dtype=torch.float32, device=dev) if X is None else X
+    R = torch.empty(B, N, dtype=torch.float32, device=dev) if R is None else R
+    n_iter = torch.empty(B, dtype=torch.int32, device=dev) if n_iter is None else n_iter
+    workspace, wp, wb = _workspace(N, M, B, workspace, dev)
+    with torch.cuda.device(dev):
+        _check(lib.mp_recover_batched(p, N, M, ld, Y.data_ptr(), ldy, B, float(eps), int(max_iter),
+                                      _dev(X, torch.float32, "X"), _dev(R, torch.float32, "R"),
+                                      _dev(n_iter, torch.int32, "n_iter"), wp, wb, _stream_ptr(stream)))
+    return Recovered(X, R, n_iter, None, None, workspace)
+
+
+def _host(t: torch.Tensor, dtype, what: str):
+    if t.is_cuda or t.dtype != dtype or not t.is_contiguous():
+        raise TypeError(f"{what} must be a contiguous CPU {dtype} tensor")
+    return t.data_ptr()
+
+
+def mp_recover_host(psi_t: torch.Tensor, y: torch.Tensor, eps: float, max_iter: int, *, normalize: bool = False,
+                    trace: bool = False, device: int = 0) -> Recovered:
+    """HOST tensors in, HOST tensors out (copies, kernels and the final synchronise inside the C call)."""
+    M, N = psi_t.shape
+    x = torch.empty(M, dtype=torch.float32).pin_memory()
+    r = torch.empty(N, dtype=torch.float32).pin_memory()
+    n_iter = torch.zeros(1, dtype=torch.int32).pin_memory()
+    it = torch.empty(max(max_iter, 1), dtype=torch.int32) if trace else None
+    ct = torch.empty(max(max_iter, 1), dtype=torch.float32) if trace else None
+    with torch.cuda.device(device):
+        _check(lib.mp_recover_host(_host(psi_t, torch.float32, "psi_t"), N, M, psi_t.stride(0) if M > 1 else N,
+                                   int(normalize), _host(y, torch.float32, "y"), float(eps), int(max_iter),
+                                   x.data_ptr(), r.data_ptr(), n_iter.data_ptr(),
+                                   it.data_ptr() if trace else None, ct.data_ptr() if trace else None))
+    return Recovered(x, r, n_iter, it, ct, None)
+
+
+def mp_recover_batched_host(psi_t: torch.Tensor, Y: torch.Tensor, eps: float, max_iter: int, *,
+                            normalize: bool = False, device: int = 0) -> Recovered:
+    M, N = psi_t.shape
+    B = Y.shape[0]
+    X = torch.empty(B, M, dtype=torch.float32).pin_memory()
+    R = torch.empty(B, N, dtype=torch.float32).pin_memory()
+    n_iter = torch.zeros(B, dtype=torch.int32).pin_memory()
+    with torch.cuda.device(device):
+        _check(lib.mp_recover_batched_host(_host(psi_t, torch.float32, "psi_t"), N, M, psi_t.stride(0) if M > 1 else N,
+                                           int(normalize), _host(Y, torch.float32, "Y"), N, B, float(eps), int(max_iter),
+                                           X.data_ptr(), R.data_ptr(), n_iter.data_ptr()))
+    return Recovered(X, R, n_iter, None, None, None)

@@ -1,0 +1,290 @@
+// mp_api.cu -- the C ABI of libmp_b200.so (include/mp_b200.h): argument validation, workspace layout,
+// algorithm dispatch, knobs, and the host-buffer convenience entry points.
+#include <atomic>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+
+#include "mp_internal.h"
+
+namespace mp {
+
+static thread_local char g_err[512] = "";
+
+mp_status fail(mp_status code, const char* fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+mp_status cuda_fail(cudaError_t e, const char* what)
+{
+    return fail(MP_ERR_CUDA, "%s: %s (%s)", what, cudaGetErrorName(e), cudaGetErrorString(e));
+}
+
+Options& options()
+{
+    static Options o;
+    return o;
+}
+
+static std::atomic<int64_t> g_launches{0};
+void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+
+mp_status device_info(DeviceInfo* out)
+{
+    static thread_local DeviceInfo cache;
+    int dev = -1;
+    MP_CUDA(cudaGetDevice(&dev));
+    if (cache.device != dev) {
+        DeviceInfo d;
+        d.device = dev;
+        MP_CUDA(cudaDeviceGetAttribute(&d.sm_count, cudaDevAttrMultiProcessorCount, dev));
+        MP_CUDA(cudaDeviceGetAttribute(&d.smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+        MP_CUDA(cudaDeviceGetAttribute(&d.coop, cudaDevAttrCooperativeLaunch, dev));
+        cache = d;
+    }
+    *out = cache;
+    return MP_OK;
+}
+
+static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+size_t workspace_layout(int N, int M, int B, void* base, Workspace* ws)
+{
+    const size_t Nr = (size_t)round_up(N, 128);
+    size_t off = 0;
+    char* b = static_cast<char*>(base);
+    auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
+    const size_t o_ctrl = take(256);
+    const size_t o_x64 = take(sizeof(double) * (size_t)B * M);     // must directly follow ctrl (one memset covers both)
+    const size_t o_r64 = take(sizeof(double) * (size_t)B * Nr);
+    const size_t o_r32 = take(sizeof(float) * (size_t)B * Nr);
+    const size_t o_keys = take(sizeof(unsigned long long) * 3 * (size_t)B);
+    const size_t o_state = take(sizeof(int) * 4 * (size_t)B);
+    if (ws) {
+        ws->ctrl = reinterpret_cast<unsigned long long*>(b + o_ctrl);
+        ws->x64 = reinterpret_cast<double*>(b + o_x64);
+        ws->r64 = reinterpret_cast<double*>(b + o_r64);
+        ws->r32 = reinterpret_cast<float*>(b + o_r32);
+        ws->keys = reinterpret_cast<unsigned long long*>(b + o_keys);
+        ws->state = reinterpret_cast<int*>(b + o_state);
+        ws->bytes = off;
+    }
+    return off;
+}
+
+static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+static mp_status check_dictionary(const float* psi_t, int N, int M, int64_t ld)
+{
+    if (!psi_t) return fail(MP_ERR_INVALID_ARG, "psi_t is null");
+    if (N < 1 || M < 1) return fail(MP_ERR_INVALID_ARG, "need N >= 1 and M >= 1 (got N=%d, M=%d)", N, M);
+    if (ld < N || (ld & 3)) return fail(MP_ERR_INVALID_ARG, "need ld >= N and ld %% 4 == 0 (got ld=%lld, N=%d)", (long long)ld, N);
+    if (!aligned16(psi_t)) return fail(MP_ERR_INVALID_ARG, "psi_t must be 16-byte aligned");
+    return MP_OK;
+}
+
+}  // namespace mp
+
+namespace {
+struct DevBuf {
+    void* p = nullptr;
+    ~DevBuf() { if (p) cudaFree(p); }
+    cudaError_t alloc(size_t bytes) { return cudaMalloc(&p, bytes ? bytes : 16); }
+    template <class T> T* as() { return static_cast<T*>(p); }
+};
+struct Stream {
+    cudaStream_t s = nullptr;
+    ~Stream() { if (s) cudaStreamDestroy(s); }
+};
+}  // namespace
+
+using namespace mp;
+
+extern "C" {
+
+size_t mp_workspace_bytes(int N, int M, int B)
+{
+    if (N < 1 || M < 1 || B < 1) return 0;
+    return workspace_layout(N, M, B, nullptr, nullptr);
+}
+
+const char* mp_last_error(void) { return g_err; }
+
+int64_t mp_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+
+static int64_t* option_slot(const char* name)
+{
+    Options& o = options();
+    if (!name) return nullptr;
+    if (!strcmp(name, "algo")) return &o.algo;
+    if (!strcmp(name, "warps")) return &o.warps;
+    if (!strcmp(name, "slot_bytes")) return &o.slot_bytes;
+    if (!strcmp(name, "depth")) return &o.depth;
+    if (!strcmp(name, "grid")) return &o.grid;
+    if (!strcmp(name, "chunk")) return &o.chunk;
+    if (!strcmp(name, "batched_algo")) return &o.batched_algo;
+    return nullptr;
+}
+
+mp_status mp_set_int(const char* name, int64_t value)
+{
+    int64_t* s = option_slot(name);
+    if (!s) return fail(MP_ERR_INVALID_ARG, "unknown option '%s'", name ? name : "(null)");
+    if (value < 0) return fail(MP_ERR_INVALID_ARG, "option '%s' must be >= 0", name);
+    *s = value;
+    return MP_OK;
+}
+
+mp_status mp_get_int(const char* name, int64_t* value)
+{
+    int64_t* s = option_slot(name);
+    if (!s || !value) return fail(MP_ERR_INVALID_ARG, "unknown option or null output");
+    *value = *s;
+    return MP_OK;
+}
+
+mp_status mp_normalize_columns(float* psi_t, int N, int M, int64_t ld, float* norms_out, void* stream)
+{
+    mp_status st = check_dictionary(psi_t, N, M, ld);
+    if (st != MP_OK) return st;
+    return launch_normalize(psi_t, N, M, ld, norms_out, static_cast<cudaStream_t>(stream));
+}
+
+mp_status mp_recover(const float* psi_t, int N, int M, int64_t ld,
+                     const float* y, float eps, int max_iter,
+                     float* x, float* r, int* n_iter,
+                     int* idx_trace, float* c_trace,
+                     void* workspace, size_t workspace_bytes, void* stream)
+{
+    mp_status st = check_dictionary(psi_t, N, M, ld);
+    if (st != MP_OK) return st;
+    if (!y || !x || !r || !n_iter) return fail(MP_ERR_INVALID_ARG, "y, x, r and n_iter must be non-null");
+    if (!aligned16(y) || !aligned16(x) || !aligned16(r)) return fail(MP_ERR_INVALID_ARG, "y, x, r must be 16-byte aligned");
+    if (max_iter < 0) return fail(MP_ERR_INVALID_ARG, "max_iter must be >= 0 (got %d)", max_iter);
+    if (!(eps >= 0.0f)) return fail(MP_ERR_INVALID_ARG, "eps must be >= 0 and not NaN");
+    const size_t need = mp_workspace_bytes(N, M, 1);
+    if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 255u) || workspace_bytes < need)
+        return fail(MP_ERR_WORKSPACE, "workspace must be non-null, 256-byte aligned and >= %zu bytes (got %zu)", need, workspace_bytes);
+
+    Workspace ws;
+    workspace_layout(N, M, 1, workspace, &ws);
+    RecoverArgs a{psi_t, N, M, ld, y, eps, max_iter, x, r, n_iter, idx_trace, c_trace};
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    const int64_t algo = options().algo;
+    if (algo == 2) return launch_recover_streamloop(a, ws, s);
+    if (algo == 1) return launch_recover_persistent(a, ws, s);
+    if (persistent_supported(N, M)) return launch_recover_persistent(a, ws, s);
+    return launch_recover_streamloop(a, ws, s);
+}
+
+mp_status mp_recover_batched(const float* psi_t, int N, int M, int64_t ld,
+                             const float* Y, int64_t ldy, int B,
+                             float eps, int max_iter,
+                             float* X, float* R, int* n_iter,
+                             void* workspace, size_t workspace_bytes, void* stream)
+{
+    mp_status st = check_dictionary(psi_t, N, M, ld);
+    if (st != MP_OK) return st;
+    if (B < 1) return fail(MP_ERR_INVALID_ARG, "need B >= 1 (got %d)", B);
+    if (!Y || !X || !R || !n_iter) return fail(MP_ERR_INVALID_ARG, "Y, X, R and n_iter must be non-null");
+    if (!aligned16(Y) || !aligned16(X) || !aligned16(R)) return fail(MP_ERR_INVALID_ARG, "Y, X, R must be 16-byte aligned");
+    if (ldy < N || (ldy & 3)) return fail(MP_ERR_INVALID_ARG, "need ldy >= N and ldy %% 4 == 0");
+    if (max_iter < 0) return fail(MP_ERR_INVALID_ARG, "max_iter must be >= 0 (got %d)", max_iter);
+    if (!(eps >= 0.0f)) return fail(MP_ERR_INVALID_ARG, "eps must be >= 0 and not NaN");
+    const size_t need = mp_workspace_bytes(N, M, B);
+    if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 255u) || workspace_bytes < need)
+        return fail(MP_ERR_WORKSPACE, "workspace must be non-null, 256-byte aligned and >= %zu bytes (got %zu)", need, workspace_bytes);
+    Workspace ws;
+    workspace_layout(N, M, B, workspace, &ws);
+    BatchedArgs a{psi_t, N, M, ld, Y, ldy, B, eps, max_iter, X, R, n_iter};
+    return launch_recover_batched(a, ws, static_cast<cudaStream_t>(stream));
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// host-buffer entry points
+// ---------------------------------------------------------------------------------------------------------
+
+mp_status mp_recover_batched_host(const float* psi_t, int N, int M, int64_t ld, int normalize,
+                                  const float* Y, int64_t ldy, int B, float eps, int max_iter,
+                                  float* X, float* R, int* n_iter)
+{
+    if (!psi_t || !Y || !X || !R || !n_iter) return fail(MP_ERR_INVALID_ARG, "null host pointer");
+    if (N < 1 || M < 1 || B < 1 || ld < N || (ld & 3) || ldy < N || (ldy & 3) || max_iter < 0 || !(eps >= 0.0f))
+        return fail(MP_ERR_INVALID_ARG, "invalid sizes");
+    Stream st;
+    MP_CUDA(cudaStreamCreateWithFlags(&st.s, cudaStreamNonBlocking));
+    DevBuf d_psi, d_Y, d_X, d_R, d_n, d_ws;
+    const size_t wsb = mp_workspace_bytes(N, M, B);
+    MP_CUDA(d_psi.alloc(sizeof(float) * (size_t)M * ld));
+    MP_CUDA(d_Y.alloc(sizeof(float) * (size_t)B * ldy));
+    MP_CUDA(d_X.alloc(sizeof(float) * (size_t)B * M));
+    MP_CUDA(d_R.alloc(sizeof(float) * (size_t)B * N));
+    MP_CUDA(d_n.alloc(sizeof(int) * (size_t)B));
+    MP_CUDA(d_ws.alloc(wsb));
+    MP_CUDA(cudaMemcpyAsync(d_psi.p, psi_t, sizeof(float) * (size_t)M * ld, cudaMemcpyHostToDevice, st.s));
+    MP_CUDA(cudaMemcpyAsync(d_Y.p, Y, sizeof(float) * (size_t)B * ldy, cudaMemcpyHostToDevice, st.s));
+    mp_status rc;
+    if (normalize) {
+        rc = mp_normalize_columns(d_psi.as<float>(), N, M, ld, nullptr, st.s);
+        if (rc != MP_OK) return rc;
+    }
+    rc = mp_recover_batched(d_psi.as<float>(), N, M, ld, d_Y.as<float>(), ldy, B, eps, max_iter,
+                            d_X.as<float>(), d_R.as<float>(), d_n.as<int>(), d_ws.p, wsb, st.s);
+    if (rc != MP_OK) return rc;
+    MP_CUDA(cudaMemcpyAsync(X, d_X.p, sizeof(float) * (size_t)B * M, cudaMemcpyDeviceToHost, st.s));
+    MP_CUDA(cudaMemcpyAsync(R, d_R.p, sizeof(float) * (size_t)B * N, cudaMemcpyDeviceToHost, st.s));
+    MP_CUDA(cudaMemcpyAsync(n_iter, d_n.p, sizeof(int) * (size_t)B, cudaMemcpyDeviceToHost, st.s));
+    MP_CUDA(cudaStreamSynchronize(st.s));
+    return MP_OK;
+}
+
+mp_status mp_recover_host(const float* psi_t, int N, int M, int64_t ld, int normalize,
+                          const float* y, float eps, int max_iter,
+                          float* x, float* r, int* n_iter, int* idx_trace, float* c_trace)
+{
+    if (!psi_t || !y || !x || !r || !n_iter) return fail(MP_ERR_INVALID_ARG, "null host pointer");
+    if (N < 1 || M < 1 || ld < N || (ld & 3) || max_iter < 0 || !(eps >= 0.0f))
+        return fail(MP_ERR_INVALID_ARG, "invalid sizes");
+    Stream st;
+    MP_CUDA(cudaStreamCreateWithFlags(&st.s, cudaStreamNonBlocking));
+    DevBuf d_psi, d_y, d_x, d_r, d_n, d_ws, d_it, d_ct;
+    const size_t wsb = mp_workspace_bytes(N, M, 1);
+    MP_CUDA(d_psi.alloc(sizeof(float) * (size_t)M * ld));
+    MP_CUDA(d_y.alloc(sizeof(float) * (size_t)N));
+    MP_CUDA(d_x.alloc(sizeof(float) * (size_t)M));
+    MP_CUDA(d_r.alloc(sizeof(float) * (size_t)N));
+    MP_CUDA(d_n.alloc(sizeof(int)));
+    MP_CUDA(d_ws.alloc(wsb));
+    if (idx_trace) MP_CUDA(d_it.alloc(sizeof(int) * (size_t)max_iter));
+    if (c_trace) MP_CUDA(d_ct.alloc(sizeof(float) * (size_t)max_iter));
+    MP_CUDA(cudaMemcpyAsync(d_psi.p, psi_t, sizeof(float) * (size_t)M * ld, cudaMemcpyHostToDevice, st.s));
+    MP_CUDA(cudaMemcpyAsync(d_y.p, y, sizeof(float) * (size_t)N, cudaMemcpyHostToDevice, st.s));
+    mp_status rc;
+    if (normalize) {
+        rc = mp_normalize_columns(d_psi.as<float>(), N, M, ld, nullptr, st.s);
+        if (rc != MP_OK) return rc;
+    }
+    rc = mp_recover(d_psi.as<float>(), N, M, ld, d_y.as<float>(), eps, max_iter, d_x.as<float>(), d_r.as<float>(),
+                    d_n.as<int>(), idx_trace ? d_it.as<int>() : nullptr, c_trace ? d_ct.as<float>() : nullptr,
+                    d_ws.p, wsb, st.s);
+    if (rc != MP_OK) return rc;
+    MP_CUDA(cudaMemcpyAsync(x, d_x.p, sizeof(float) * (size_t)M, cudaMemcpyDeviceToHost, st.s));
+    MP_CUDA(cudaMemcpyAsync(r, d_r.p, sizeof(float) * (size_t)N, cudaMemcpyDeviceToHost, st.s));
+    MP_CUDA(cudaMemcpyAsync(n_iter, d_n.p, sizeof(int), cudaMemcpyDeviceToHost, st.s));
+    MP_CUDA(cudaStreamSynchronize(st.s));
+    if (idx_trace || c_trace) {
+        const int t = *n_iter;
+        if (idx_trace && t > 0) MP_CUDA(cudaMemcpyAsync(idx_trace, d_it.p, sizeof(int) * (size_t)t, cudaMemcpyDeviceToHost, st.s));
+        if (c_trace && t > 0) MP_CUDA(cudaMemcpyAsync(c_trace, d_ct.p, sizeof(float) * (size_t)t, cudaMemcpyDeviceToHost, st.s));
+        MP_CUDA(cudaStreamSynchronize(st.s));
+    }
+    return MP_OK;
+}
+
+}  // extern "C"

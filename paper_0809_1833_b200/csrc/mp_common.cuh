@@ -1,0 +1,142 @@
+// mp_common.cuh -- shared device helpers of the B200 Matching Pursuit kernels (sm_100a).
+// Product code: shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace mp {
+
+// ------------------------------------------------------------------------------------------------
+// Packed argmax key (Eq. 9 / Eq. 16: largest |c|, smallest index on ties).
+//   bits 63..32  float bits of |c|   (|c| >= 0, so IEEE bits order as unsigned ints; NaN -> 0)
+//   bits 31..1   0x7FFFFFFF - index  (lower index = larger key)
+//   bit  0       sign bit of c       (rides along so the signed c is recovered without a second read)
+// max() over keys is exact and order-independent, so a block/grid reduction by atomicMax is deterministic.
+// Every real key is > 0 (index < 0x7FFFFFFF), so 0 is the "empty" value of a key slot.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned long long pack_key(float c, int index)
+{
+    unsigned int bits = __float_as_uint(c);
+    unsigned int mag = bits & 0x7FFFFFFFu;
+    if (mag > 0x7F800000u) mag = 0u;                       // NaN never wins
+    unsigned int lo = ((0x7FFFFFFFu - (unsigned int)index) << 1) | (bits >> 31);
+    return ((unsigned long long)mag << 32) | lo;
+}
+__device__ __forceinline__ int key_index(unsigned long long key)
+{
+    return (int)(0x7FFFFFFFu - ((unsigned int)(key & 0xFFFFFFFFull) >> 1));
+}
+__device__ __forceinline__ float key_value(unsigned long long key)
+{
+    unsigned int mag = (unsigned int)(key >> 32);
+    unsigned int sign = (unsigned int)(key & 1ull) << 31;
+    return __uint_as_float(mag | sign);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Warp reductions.  xor-butterflies with a commutative op leave the bit-identical result in every lane.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ float warp_sum(float v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+__device__ __forceinline__ unsigned long long warp_max(unsigned long long v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        unsigned long long w = __shfl_xor_sync(0xffffffffu, v, o);
+        v = w > v ? w : v;
+    }
+    return v;
+}
+
+// ------------------------------------------------------------------------------------------------
+// mbarrier + TMA bulk-copy PTX (sm_90+/sm_100a).  SASS: SYNCS.*, UBLKCP.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p)
+{
+    return (uint32_t)__cvta_generic_to_shared(p);
+}
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_fence_init()
+{
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity)
+{
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
+{
+    while (!mbar_try_wait(bar, parity)) {}
+}
+// generic-proxy accesses to shared memory before this fence are ordered before later async-proxy (TMA) accesses
+__device__ __forceinline__ void fence_proxy_async_smem()
+{
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+// 1-D bulk copy global -> shared, completion reported on an mbarrier (bytes % 16 == 0, 16-B aligned both sides)
+__device__ __forceinline__ void tma_load_1d(void* smem_dst, const void* gmem_src, uint32_t bytes, uint64_t* bar)
+{
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+        ::"r"(smem_u32(smem_dst)), "l"(gmem_src), "r"(bytes), "r"(smem_u32(bar))
+        : "memory");
+}
+
+// ------------------------------------------------------------------------------------------------
+// gpu-scope atomics / ordered accesses used by the grid barrier
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void red_max_u64(unsigned long long* p, unsigned long long v)
+{
+    asm volatile("red.relaxed.gpu.global.max.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+__device__ __forceinline__ void red_add_release_u64(unsigned long long* p, unsigned long long v)
+{
+    asm volatile("red.release.gpu.global.add.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+__device__ __forceinline__ unsigned long long ld_acquire_u64(const unsigned long long* p)
+{
+    unsigned long long v;
+    asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ unsigned long long ld_relaxed_u64(const unsigned long long* p)
+{
+    unsigned long long v;
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_relaxed_u64(unsigned long long* p, unsigned long long v)
+{
+    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+__device__ __forceinline__ void red_add_f64(double* p, double v)
+{
+    asm volatile("red.relaxed.gpu.global.add.f64 [%0], %1;" ::"l"(p), "d"(v) : "memory");
+}
+
+}  // namespace mp

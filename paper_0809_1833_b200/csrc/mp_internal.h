@@ -1,0 +1,67 @@
+// mp_internal.h -- host-side plumbing shared by the translation units of libmp_b200.so.
+#pragma once
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include <stdint.h>
+
+#include "../../include/mp_b200.h"
+
+namespace mp {
+
+// ---- error reporting (thread-local message behind mp_last_error) --------------------------------------
+mp_status fail(mp_status code, const char* fmt, ...);
+mp_status cuda_fail(cudaError_t e, const char* what);
+#define MP_CUDA(call)                                                   \
+    do {                                                                \
+        cudaError_t e__ = (call);                                       \
+        if (e__ != cudaSuccess) return ::mp::cuda_fail(e__, #call);     \
+    } while (0)
+
+// ---- process-wide knobs (mp_set_int) ---------------------------------------------------------------------
+struct Options {
+    int64_t algo = 0, warps = 0, slot_bytes = 0, depth = 0, grid = 0, chunk = 64;
+    int64_t batched_algo = 0;
+};
+Options& options();
+void count_launch(int n = 1);
+
+// ---- device info (cached per device) ---------------------------------------------------------------------
+struct DeviceInfo {
+    int device = -1, sm_count = 0, smem_optin = 0, coop = 0;
+};
+mp_status device_info(DeviceInfo* out);
+
+// ---- workspace layout --------------------------------------------------------------------------------------
+// [ctrl: 256 B][x64: B*M doubles][r64: B*Nr doubles][r32: B*Nr floats][keys: B u64, padded][flags ...]
+struct Workspace {
+    unsigned long long* ctrl;   // [0] grid-barrier counter, [1..3] rotating key slots (single), [4] done flag, [8..] misc
+    double* x64;                // B*M
+    double* r64;                // B*Nr   (Nr = N rounded up to 128)
+    float* r32;                 // B*Nr
+    unsigned long long* keys;   // 3*B  rotating per-signal key slots (batched)
+    int* state;                 // B    per-signal: 1 = active
+    size_t bytes;
+};
+size_t workspace_layout(int N, int M, int B, void* base, Workspace* ws);
+static inline int round_up(int v, int m) { return (v + m - 1) / m * m; }
+
+// ---- launchers (each enqueues on `stream`, returns MP_OK or an error) ---------------------------------------
+mp_status launch_normalize(float* psi_t, int N, int M, int64_t ld, float* norms_out, cudaStream_t stream);
+
+struct RecoverArgs {
+    const float* psi_t; int N, M; int64_t ld;
+    const float* y; float eps; int max_iter;
+    float* x; float* r; int* n_iter; int* idx_trace; float* c_trace;
+};
+mp_status launch_recover_persistent(const RecoverArgs& a, const Workspace& ws, cudaStream_t stream);
+bool persistent_supported(int N, int M);
+mp_status launch_recover_streamloop(const RecoverArgs& a, const Workspace& ws, cudaStream_t stream);
+
+struct BatchedArgs {
+    const float* psi_t; int N, M; int64_t ld;
+    const float* Y; int64_t ldy; int B; float eps; int max_iter;
+    float* X; float* R; int* n_iter;
+};
+mp_status launch_recover_batched(const BatchedArgs& a, const Workspace& ws, cudaStream_t stream);
+
+}  // namespace mp

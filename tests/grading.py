@@ -1,0 +1,164 @@
+"""Grading of a GPU Matching Pursuit run against the CPU oracle (test infrastructure).
+
+Implements the parity contract of BASELINE.json's north_star under the readings listed in DESIGN.md:
+
+  G1 free-running: the GPU index sequence equals the oracle's up to the first iteration whose top-two
+     relative gap of |c| (on the oracle's own state) is <= 1e-4 -- after a legal near-tie flip the two
+     runs are different trajectories and cannot be compared step by step.
+  G2 teacher-forced replay over the WHOLE GPU trace: the oracle is advanced with the GPU's own (index,
+     step) pairs, so its state is the exact-arithmetic image of the GPU state; at every iteration the
+     GPU's pick must be the oracle's argmax, or a near-tie (gap <= 1e-4 and |c_ref[pick]| >= (1-1e-4) max).
+  G3 every step value: |c_gpu - c_ref[pick]| <= C_TOL * ||r_t||  (fp32 dot product of N terms against a
+     float64 reference; bound derived in DESIGN.md "Tolerances").
+  G4 final residual: | ||r_gpu|| - ||r_replay|| | <= 1e-4 ||r_replay||  (north_star) -- and, tighter,
+     the vector itself to fp32 rounding;  x_gpu equals the replay's x to fp32 rounding.
+  G5 stop rule: the GPU continued exactly while ||r|| > eps ||y|| and t < T, judged on the replay's norms.
+  G6 exact-recovery regime (oracle stops by eps with ||x_ref - x_true|| <= 1e-4 ||x_true||): selected atoms
+     == true support, ||x_gpu - x_ref|| <= 1e-4 ||x_ref||.
+"""
+from __future__ import annotations
+
+import dataclasses
+
+import numpy as np
+
+import oracle
+
+GAP_TOL = 1e-4      # north_star: "top-two |c| gap exceeds 1e-4 relative"
+C_TOL = 4e-6        # |c_gpu - c_ref| / ||r_t||, see DESIGN.md "Tolerances"
+NORM_TOL = 1e-4     # north_star: final ||r|| within 1e-4 relative
+X_TOL = 1e-4        # north_star: ||x_gpu - x_ref|| / ||x_ref||
+
+
+@dataclasses.dataclass
+class Grade:
+    n_iter_gpu: int
+    n_iter_ref: int
+    first_divergence: int          # -1 if the free-running sequences agree on their common prefix
+    near_ties: int                 # iterations with gap <= GAP_TOL (replay)
+    flips: int                     # iterations where the GPU pick != oracle argmax (all legal if we got here)
+    max_c_err: float               # max |c_gpu - c_ref| / ||r_t||
+    rnorm_rel_err: float
+    x_rel_err_vs_ref: float
+    exact_recovery: bool
+
+
+def grade_single(psi32: np.ndarray, y32: np.ndarray, eps: float, max_iter: int,
+                 x_gpu, r_gpu, n_iter_gpu, idx_gpu, c_gpu, *, x_true=None, support=None,
+                 nthreads: int | None = None, ref: "oracle.MPResult | None" = None) -> Grade:
+    nthreads = nthreads or oracle.default_threads()
+    eps = float(np.float32(eps))                       # the very float the GPU received
+    y = y32.astype(np.float64)
+    t_gpu = int(n_iter_gpu)
+    idx_gpu = np.asarray(idx_gpu[:t_gpu], dtype=np.int32)
+    c_gpu = np.asarray(c_gpu[:t_gpu], dtype=np.float64)
+    x_gpu = np.asarray(x_gpu, dtype=np.float64)
+    r_gpu = np.asarray(r_gpu, dtype=np.float64)
+    M, N = psi32.shape
+    assert 0 <= t_gpu <= max_iter
+    assert np.all((idx_gpu >= 0) & (idx_gpu < M)), "index out of range"
+
+    if ref is None:
+        ref = oracle.mp(psi32, y, eps, max_iter, nthreads)
+    ny = ref.rnorm[0] if ref.rnorm.size else 0.0
+
+    # ---- G1 free-running ------------------------------------------------------------------------------
+    L = min(t_gpu, ref.n_iter)
+    diff = np.nonzero(idx_gpu[:L] != ref.idx[:L])[0]
+    first_div = int(diff[0]) if diff.size else -1
+    if first_div >= 0:
+        assert ref.gap[first_div] <= GAP_TOL, (
+            f"free-running sequences diverge at t={first_div} where the oracle's top-two gap is {ref.gap[first_div]:.3e} > {GAP_TOL}")
+
+    # ---- G2/G3 teacher-forced replay ------------------------------------------------------------------------
+    rp = oracle.mp_replay(psi32, y, idx_gpu, c_gpu, nthreads)
+    same = idx_gpu == rp.argmax_ref
+    legal = same | ((rp.gap <= GAP_TOL) & (np.abs(rp.c_at_idx) >= (1.0 - GAP_TOL) * rp.cmax_ref))
+    bad = np.nonzero(~legal)[0]
+    assert bad.size == 0, (
+        f"{bad.size} illegal picks, first at t={bad[0]}: gpu idx {idx_gpu[bad[0]]} |c_ref|={abs(rp.c_at_idx[bad[0]]):.9e} "
+        f"vs oracle idx {rp.argmax_ref[bad[0]]} max={rp.cmax_ref[bad[0]]:.9e} gap={rp.gap[bad[0]]:.3e}")
+    c_err = np.abs(c_gpu - rp.c_at_idx) / np.maximum(rp.rnorm[:t_gpu], np.finfo(np.float64).tiny) if t_gpu else np.zeros(0)
+    max_c_err = float(c_err.max()) if t_gpu else 0.0
+    assert max_c_err <= C_TOL, f"step value error {max_c_err:.3e} ||r|| at t={int(c_err.argmax())} exceeds {C_TOL}"
+
+    # ---- G4 final residual and coefficients ---------------------------------------------------------------------
+    nr_gpu = float(np.linalg.norm(r_gpu))
+    nr_rep = float(rp.rnorm[t_gpu])
+    rn_err = abs(nr_gpu - nr_rep) / nr_rep if nr_rep > 0 else abs(nr_gpu)
+    assert rn_err <= NORM_TOL, f"final ||r|| off by {rn_err:.3e} relative"
+    assert np.linalg.norm(r_gpu - rp.r) <= 1.2e-7 * np.linalg.norm(rp.r) + 1e-30, "r is not the fp32 rounding of y - Psi x~"
+    assert np.all(np.abs(x_gpu - rp.x) <= 6e-8 * np.abs(rp.x) + 1e-45), "x is not the fp32 rounding of the accumulated steps"
+
+    # ---- G5 stop rule ------------------------------------------------------------------------------------------------
+    thr = eps * ny
+    if t_gpu:
+        assert np.all(rp.rnorm[:t_gpu] > thr * (1.0 - 1e-9)), "GPU continued although ||r|| <= eps ||y||"
+    if t_gpu < max_iter:
+        assert rp.rnorm[t_gpu] <= thr * (1.0 + 1e-9), "GPU stopped although ||r|| > eps ||y|| and t < T"
+
+    # ---- n_iter --------------------------------------------------------------------------------------------------------
+    if first_div < 0:
+        if t_gpu != ref.n_iter:
+            # only a rounding-level tie at the stopping threshold may move n_iter by one
+            assert abs(t_gpu - ref.n_iter) == 1, f"n_iter {t_gpu} vs oracle {ref.n_iter} on identical sequences"
+            edge = ref.rnorm[min(t_gpu, ref.n_iter)]
+            assert abs(edge - thr) <= NORM_TOL * thr, "n_iter differs by one away from the stopping threshold"
+
+    # ---- G6 exact-recovery regime -----------------------------------------------------------------------------------------
+    x_err_ref = float(np.linalg.norm(x_gpu - ref.x) / max(np.linalg.norm(ref.x), 1e-300)) if ref.n_iter else 0.0
+    exact = False
+    if x_true is not None and ref.n_iter < max_iter and np.linalg.norm(ref.x - x_true) <= X_TOL * np.linalg.norm(x_true):
+        exact = True
+        assert x_err_ref <= X_TOL, f"||x_gpu - x_ref||/||x_ref|| = {x_err_ref:.3e}"
+        assert t_gpu < max_iter and np.linalg.norm(r_gpu) <= thr * (1 + 1e-6)
+        if support is not None:
+            sup = set(int(s) for s in support)
+            if set(ref.idx.tolist()) == sup:           # strict form holds for the oracle -> must hold for the GPU
+                assert set(idx_gpu.tolist()) == sup, "selected atoms differ from the true support"
+            tau = 1e-3 * np.max(np.abs(x_true))
+            off = np.ones(M, bool); off[list(sup)] = False
+            assert not np.any(np.abs(x_gpu[off]) > tau), "off-support coefficient above tau"
+            big = [m for m in sup if abs(x_true[m]) >= 2 * tau]
+            assert np.all(np.abs(x_gpu[big]) > tau), "a true coefficient is missing"
+    return Grade(t_gpu, ref.n_iter, first_div, int(np.sum(rp.gap <= GAP_TOL)), int(np.sum(~same)),
+                 max_c_err, rn_err, x_err_ref, exact)
+
+
+def residual_at(psi32: np.ndarray, y32: np.ndarray, idx, c, t: int) -> np.ndarray:
+    """y - sum_{s<t} c_s psi_{idx_s} in float64: the exact-arithmetic image of the run's state before step t."""
+    r = y32.astype(np.float64).copy()
+    idx = np.asarray(idx[:t]); c = np.asarray(c[:t], dtype=np.float64)
+    if t:
+        coef = np.zeros(psi32.shape[0]); np.add.at(coef, idx, c)
+        for m in np.nonzero(coef)[0]:
+            r -= coef[m] * psi32[m].astype(np.float64)
+    return r
+
+
+def grade_sampled(psi32, y32, idx_gpu, c_gpu, n_iter_gpu, r_gpu, sample_ts, nthreads=None):
+    """Full-size check on SAMPLED iterations the oracle can compute one by one: for each t in sample_ts the
+    state is rebuilt in float64 from the GPU trace, one oracle correlation pass gives c_ref, and the GPU's pick
+    and step must satisfy G2/G3.  Also checks the final residual (G4)."""
+    nthreads = nthreads or oracle.default_threads()
+    t_gpu = int(n_iter_gpu)
+    out = []
+    for t in sample_ts:
+        if not 0 <= t < t_gpu:
+            continue
+        r = residual_at(psi32, y32, idx_gpu, c_gpu, t)
+        c = oracle.correlate(psi32, r, nthreads)
+        i_ref = oracle.argmax_abs(c)
+        a = np.abs(c); a1 = a[i_ref]
+        a2 = np.max(np.delete(a, i_ref)) if a.size > 1 else 0.0
+        gap = (a1 - a2) / a1 if a1 > 0 else 0.0
+        i = int(idx_gpu[t])
+        assert i == i_ref or (gap <= GAP_TOL and a[i] >= (1 - GAP_TOL) * a1), f"illegal pick at sampled t={t}"
+        err = abs(float(c_gpu[t]) - c[i]) / oracle.nrm2(r)
+        assert err <= C_TOL, f"step value error {err:.3e} at sampled t={t}"
+        out.append((t, gap, err))
+    r_fin = residual_at(psi32, y32, idx_gpu, c_gpu, t_gpu)
+    nr = oracle.nrm2(r_fin)
+    assert abs(np.linalg.norm(np.asarray(r_gpu, np.float64)) - nr) <= NORM_TOL * nr
+    assert np.linalg.norm(np.asarray(r_gpu, np.float64) - r_fin) <= 1.2e-7 * nr + 1e-30
+    return out
