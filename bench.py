@@ -1,0 +1,312 @@
+#!/usr/bin/env python
+"""bench.py -- Matching Pursuit on B200: MP iterations/s and achieved HBM GB/s vs the measured peak.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config cfg3] [--impl reference]
+
+One "step" = one pass of the whole hot path over one synthetic problem: column
+normalisation of the dictionary (a0) followed by one complete mp_recover solve (a1-a8: init, the device-resident
+loop of fused correlate+argmax / update+norm / stop test, return of x~, r, n_iter).  The default workload is
+BASELINE.json's metric configuration (configs[2] = "cfg3": N=4096, M=16384 fp32 Bernoulli dictionary, K=256).
+The dictionary (256 MiB) is larger than L2 (126 MB), so every MP iteration streams it from HBM: no L2 flush is
+needed between timed iterations (stated in config.l2).
+
+Prints ONE JSON line (rank 0).  Multi-GPU (torchrun): the path does not shard ("replicas only"):
+every rank solves its own problem of the same shape; value = iterations of all ranks / max-over-ranks time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_0809_1833_b200 import synth  # noqa: E402  (seeded inputs only; numpy)
+
+METRIC = "mp_iterations_per_s"
+UNIT = "iterations/s"
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            d = json.load(open(p))
+            return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def ncu_traffic_per_iteration():
+    """DRAM bytes per MP iteration of the dominant kernel from the committed ncu capture, or None."""
+    p = os.path.join(ROOT, "profiles", "dominant_kernel_traffic.txt")
+    try:
+        for line in open(p):
+            if line.startswith("dram_bytes_per_iteration"):
+                return float(line.split("=")[1].split()[0])
+    except Exception:
+        pass
+    return None
+
+
+class ClockSampler:
+    """nvidia-smi clocks/throttle reasons DURING the timed region (B200_PROFILING.md clocks line)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, mx, reasons = [], None, set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx = float(r[1])
+            except Exception:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def build_problem(cfg: synth.Config, seed: int):
+    """Host-side seeded inputs.  Returns raw dictionary [M,N] fp32 and Y [B,N] fp32.
+    y = Psi x is formed from the dictionary the solver will see; for Gaussian configs the columns are normalised
+    on the DEVICE by the product kernel before encoding, so this returns (psi_raw, X, S) and the caller encodes."""
+    psi_raw = synth.make_dictionary(cfg, seed)
+    X = np.zeros((cfg.B, cfg.M)); S = np.zeros((cfg.B, cfg.K), dtype=np.int64)
+    for b in range(cfg.B):
+        X[b], S[b] = synth.sparse_signal(cfg.M, cfg.K, seed, cfg.values, signal=b)
+    return psi_raw, X, S
+
+
+def run_reference(args, cfg):
+    """--impl reference: the CPU oracle, as it stands, on the box's host cores; each step = a bounded sample
+    (max_iter capped) of the same workload."""
+    import oracle
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    import problems
+    pb = problems.make_problem(cfg, seed=1)
+    threads = oracle.default_threads()
+    y = pb.Y[0].astype(np.float64)
+    t0 = time.perf_counter(); oracle.mp(pb.psi32, y, cfg.eps, 4, threads); per_it = (time.perf_counter() - t0) / 4
+    budget = 150.0 / max(1, args.steps + args.warmup)
+    T = int(max(4, min(cfg.max_iter, budget / per_it)))
+    for _ in range(args.warmup):
+        oracle.mp(pb.psi32, y, cfg.eps, T, threads)
+    t0 = time.perf_counter(); its = 0
+    for _ in range(args.steps):
+        its += oracle.mp(pb.psi32, y, cfg.eps, T, threads).n_iter
+    dt = time.perf_counter() - t0
+    v = its / dt
+    sample = f"first {T} MP iterations of {cfg.name} per step (float64 C oracle, OpenMP over atoms)"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(cfg), "sample": sample},
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+        "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def workload_name(cfg):
+    return (f"{cfg.name}: single-signal MP fp32, N={cfg.N}, M={cfg.M}, K={cfg.K}, {cfg.dictionary} dictionary, "
+            f"eps={cfg.eps:g}, max_iter={cfg.max_iter}" + (f", B={cfg.B}" if cfg.B > 1 else ""))
+
+
+def cpu_baseline(cfg, psi32, y32):
+    """The oracle as it stands on this box's host cores, bounded sample (about 10-20 s)."""
+    import oracle
+    threads = oracle.default_threads()
+    y = y32.astype(np.float64)
+    t0 = time.perf_counter(); oracle.mp(psi32, y, cfg.eps, 4, threads); per_it = (time.perf_counter() - t0) / 4
+    T = int(max(4, min(cfg.max_iter, 12.0 / per_it)))
+    t0 = time.perf_counter(); res = oracle.mp(psi32, y, cfg.eps, T, threads); dt = time.perf_counter() - t0
+    return {"value": res.n_iter / dt, "unit": UNIT, "cores": threads, "kind": "oracle",
+            "sample": f"first {res.n_iter} MP iterations of {cfg.name} (float64 C oracle, OpenMP over atoms, {threads} threads)"}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="cfg3")
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--max-iter", type=int, default=None, help="override the config's iteration cap (profiling runs)")
+    args = ap.parse_args()
+    cfg = synth.config(args.config)
+    if args.max_iter is not None:
+        cfg = synth.Config(**{**cfg.__dict__, "max_iter": args.max_iter})
+    if args.impl == "reference":
+        return run_reference(args, cfg)
+    if args.warmup < 3:
+        print("note: warmup < 3 breaks the timing rules; use only for profiling runs", file=sys.stderr)
+
+    import torch
+    import paper_0809_1833_b200 as mp   # raises if the CUDA library is missing: there is no fallback
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = torch.device("cuda", local)
+
+    # ---- inputs: seeded, synthetic, resident in HBM before the timed region ---------------------------------
+    psi_raw, X, S = build_problem(cfg, seed=1 + rank)
+    psi_d = torch.from_numpy(psi_raw).to(dev)
+    mp.mp_normalize_columns(psi_d)                       # so y can be encoded from the bits the solver sees
+    torch.cuda.synchronize()
+    psi32 = psi_d.cpu().numpy() if cfg.dictionary == "gaussian" else psi_raw
+    Y = np.stack([synth.encode(psi32, X[b], S[b]) for b in range(cfg.B)])
+    y_d = torch.from_numpy(Y).to(dev)
+    N, M, B = cfg.N, cfg.M, cfg.B
+    stream = torch.cuda.current_stream()
+    ws = torch.empty(mp.mp_workspace_bytes(N, M, B) + 256, dtype=torch.uint8, device=dev)
+    x_d = torch.empty(B, M, dtype=torch.float32, device=dev)
+    r_d = torch.empty(B, N, dtype=torch.float32, device=dev)
+    n_d = torch.empty(B, dtype=torch.int32, device=dev)
+
+    def step():
+        mp.mp_normalize_columns(psi_d)                                               # a0 (idempotent on unit columns)
+        if B == 1:
+            mp.mp_recover(psi_d, y_d[0], cfg.eps, cfg.max_iter, x=x_d[0], r=r_d[0], n_iter=n_d, workspace=ws)
+        else:
+            mp.mp_recover_batched(psi_d, y_d, cfg.eps, cfg.max_iter, X=x_d, R=r_d, n_iter=n_d, workspace=ws)
+
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+    its_per_step = int(n_d.sum().item()) if args.warmup else None
+
+    # ---- timed region: K steps, CUDA events on the launching stream, barrier + sync on both sides --------------
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2 * args.steps + 2)]
+    clocks = ClockSampler(local); clocks.start()
+    if dist: dist.barrier()
+    torch.cuda.synchronize()
+    l0 = mp.mp_launch_count()
+    ev[0].record(stream)
+    for k in range(args.steps):
+        mp.mp_normalize_columns(psi_d)
+        ev[2 + 2 * k].record(stream)
+        if B == 1:
+            mp.mp_recover(psi_d, y_d[0], cfg.eps, cfg.max_iter, x=x_d[0], r=r_d[0], n_iter=n_d, workspace=ws)
+        else:
+            mp.mp_recover_batched(psi_d, y_d, cfg.eps, cfg.max_iter, X=x_d, R=r_d, n_iter=n_d, workspace=ws)
+        ev[3 + 2 * k].record(stream)
+    ev[1].record(stream)
+    torch.cuda.synchronize()
+    if dist: dist.barrier()
+    launches = mp.mp_launch_count() - l0
+    clk = clocks.stop()
+    ms_total = ev[0].elapsed_time(ev[1])
+    ms_solve = [ev[2 + 2 * k].elapsed_time(ev[3 + 2 * k]) for k in range(args.steps)]
+    its_per_step = int(n_d.sum().item())
+    its_max = int(n_d.max().item())
+    t_all = torch.tensor([ms_total], dtype=torch.float64, device=dev)
+    its_all = torch.tensor([float(its_per_step * args.steps)], dtype=torch.float64, device=dev)
+    if dist:
+        dist.all_reduce(t_all, op=dist.ReduceOp.MAX)
+        dist.all_reduce(its_all, op=dist.ReduceOp.SUM)
+    ms_total_max = float(t_all.item())
+    value = float(its_all.item()) / (ms_total_max * 1e-3)
+
+    # ---- roofline of the dominant kernel (the persistent MP loop; one launch per solve) -------------------------
+    peak, peak_src = load_peaks()
+    # algorithmic bytes per launch: each iteration streams the dictionary once (4NM) and re-reads the winning atom (4N)
+    # (SURVEY.md 8(d)); the batched loop runs until its slowest signal stops.
+    alg_bytes = its_max * (4.0 * N * M + 4.0 * N * B)
+    solve_ms = float(np.mean(ms_solve))
+    achieved = alg_bytes / (solve_ms * 1e-3) / 1e9
+    per_it = ncu_traffic_per_iteration() if args.config == "cfg3" else None
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": per_it * its_max if per_it else None, "peak_source": peak_src,
+                "kernel": mp_kernel_name(mp), "algorithmic_bytes_per_launch": alg_bytes, "kernel_ms": solve_ms,
+                "us_per_iteration": 1e3 * solve_ms / max(its_max, 1)}
+
+    # ---- e2e: the host-buffer C-ABI call, H2D of the dictionary and y and D2H of x, r, n_iter inside the timed region ----
+    e2e = None
+    if not args.no_e2e and B == 1:
+        hp = torch.from_numpy(psi_raw).pin_memory(); hy = torch.from_numpy(Y[0]).pin_memory()
+        for _ in range(2):
+            mp.mp_recover_host(hp, hy, cfg.eps, cfg.max_iter, normalize=True, device=local)
+        if dist: dist.barrier()
+        t0 = time.perf_counter(); its = 0
+        for _ in range(args.steps):
+            its += int(mp.mp_recover_host(hp, hy, cfg.eps, cfg.max_iter, normalize=True, device=local).n_iter.item())
+        dt = time.perf_counter() - t0
+        t_e = torch.tensor([dt], dtype=torch.float64, device=dev); i_e = torch.tensor([float(its)], dtype=torch.float64, device=dev)
+        if dist:
+            dist.all_reduce(t_e, op=dist.ReduceOp.MAX); dist.all_reduce(i_e, op=dist.ReduceOp.SUM)
+        e2e = {"value": float(i_e.item()) / float(t_e.item()), "unit": UNIT,
+               "h2d_bytes_per_step": 4 * N * M + 4 * N, "d2h_bytes_per_step": 4 * M + 4 * N + 4,
+               "ms_per_step": 1e3 * float(t_e.item()) / args.steps,
+               "note": "mp_recover_host: cudaMalloc + H2D(Psi, y) + normalise + solve + D2H(x, r, n_iter) + free per step"}
+
+    if rank == 0:
+        cb = None
+        if not args.no_cpu_baseline and world == 1:
+            cb = cpu_baseline(cfg, psi32, Y[0])
+        print(json.dumps({
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_total_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": workload_name(cfg), "iterations_per_step": its_per_step,
+                       "step": "mp_normalize_columns + mp_recover (whole solve to the eps stop)",
+                       "l2": "dictionary 4NM = %.0f MiB > 126 MB L2: inputs larger than L2, no flush" % (4.0 * N * M / 2**20)
+                             if 4.0 * N * M > 126e6 else "dictionary fits in L2 (cache-resident regime, by design of this config)",
+                       "parallelism": "replicas only" if world > 1 else "1 GPU"},
+            "time_to_recovery_ms": solve_ms, "gpu_launches": int(launches), "clocks": clk,
+            "roofline": roofline, "cpu_baseline": cb, "e2e": e2e}))
+    if dist:
+        dist.destroy_process_group()
+
+
+def mp_kernel_name(mp):
+    try:
+        return {0: "auto", 1: "mp_persistent_kernel", 2: "stream loop"}[mp.mp_get_int("algo")]
+    except Exception:
+        return "?"
+
+
+if __name__ == "__main__":
+    main()

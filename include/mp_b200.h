@@ -98,6 +98,16 @@ MP_API mp_status mp_recover_batched(const float* psi_t, int N, int M, int64_t ld
                              float* X, float* R, int* n_iter,
                              void* workspace, size_t workspace_bytes, void* stream);
 
+/* mp_recover_batched plus per-signal traces (both nullable): idx_trace[b*ldt + t], c_trace[b*ldt + t] for
+ * t < n_iter[b], ldt >= max_iter.  Same results bit for bit; the traces make every iteration of every signal
+ * gradable after a legal near-tie flip. */
+MP_API mp_status mp_recover_batched_traced(const float* psi_t, int N, int M, int64_t ld,
+                                    const float* Y, int64_t ldy, int B,
+                                    float eps, int max_iter,
+                                    float* X, float* R, int* n_iter,
+                                    int* idx_trace, float* c_trace, int64_t ldt,
+                                    void* workspace, size_t workspace_bytes, void* stream);
+
 /* Description of the last error on this thread ("" if none).  Static storage, never NULL. */
 MP_API const char* mp_last_error(void);
 

@@ -48,6 +48,8 @@ lib.mp_recover.restype = _i
 lib.mp_recover.argtypes = [_vp, _i, _i, _i64, _vp, _f, _i, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]
 lib.mp_recover_batched.restype = _i
 lib.mp_recover_batched.argtypes = [_vp, _i, _i, _i64, _vp, _i64, _i, _f, _i, _vp, _vp, _vp, _vp, _sz, _vp]
+lib.mp_recover_batched_traced.restype = _i
+lib.mp_recover_batched_traced.argtypes = [_vp, _i, _i, _i64, _vp, _i64, _i, _f, _i, _vp, _vp, _vp, _vp, _vp, _i64, _vp, _sz, _vp]
 lib.mp_last_error.restype = C.c_char_p
 lib.mp_last_error.argtypes = []
 lib.mp_set_int.restype = _i
@@ -161,23 +163,34 @@ def mp_recover(psi_t: torch.Tensor, y: torch.Tensor, eps: float, max_iter: int, 
 
 
 def mp_recover_batched(psi_t: torch.Tensor, Y: torch.Tensor, eps: float, max_iter: int, *, X=None, R=None, n_iter=None,
-                       workspace=None, stream=None) -> Recovered:
-    """B signals sharing psi_t: Y[B, N] -> X[B, M], R[B, N], n_iter[B]."""
+                       idx_trace=None, c_trace=None, trace: bool = False, workspace=None, stream=None) -> Recovered:
+    """B signals sharing psi_t: Y[B, N] -> X[B, M], R[B, N], n_iter[B] (+ traces [B, max_iter] if asked)."""
     p, N, M, ld = _dict_args(psi_t)
     dev = psi_t.device
-    if not (Y.is_cuda and Y.dtype == torch.float32 and Y.dim() == 2 and Y.shape[1] == N and Y.stride(1) == 1):
+    if not (Y.is_cuda and Y.dtype == torch.float32 and Y.dim() == 2 and Y.shape[1] == N and (N == 1 or Y.stride(1) == 1)):
         raise TypeError("Y must be a CUDA float32 [B, N] tensor with unit stride along N")
     B = Y.shape[0]
     ldy = Y.stride(0) if B > 1 else max(Y.stride(0), N)
     X = torch.empty(B, M, dtype=torch.float32, device=dev) if X is None else X
     R = torch.empty(B, N, dtype=torch.float32, device=dev) if R is None else R
     n_iter = torch.empty(B, dtype=torch.int32, device=dev) if n_iter is None else n_iter
+    if trace and idx_trace is None:
+        idx_trace = torch.empty(B, max(max_iter, 1), dtype=torch.int32, device=dev)
+    if trace and c_trace is None:
+        c_trace = torch.empty(B, max(max_iter, 1), dtype=torch.float32, device=dev)
+    ldt = max(max_iter, 1)
+    for t_ in (idx_trace, c_trace):
+        if t_ is not None and tuple(t_.shape) != (B, ldt):
+            raise ValueError("traces must have shape [B, max(max_iter, 1)]")
     workspace, wp, wb = _workspace(N, M, B, workspace, dev)
     with torch.cuda.device(dev):
-        _check(lib.mp_recover_batched(p, N, M, ld, Y.data_ptr(), ldy, B, float(eps), int(max_iter),
-                                      _dev(X, torch.float32, "X"), _dev(R, torch.float32, "R"),
-                                      _dev(n_iter, torch.int32, "n_iter"), wp, wb, _stream_ptr(stream)))
-    return Recovered(X, R, n_iter, None, None, workspace)
+        _check(lib.mp_recover_batched_traced(
+            p, N, M, ld, Y.data_ptr(), ldy, B, float(eps), int(max_iter),
+            _dev(X, torch.float32, "X"), _dev(R, torch.float32, "R"), _dev(n_iter, torch.int32, "n_iter"),
+            _dev(idx_trace, torch.int32, "idx_trace") if idx_trace is not None else None,
+            _dev(c_trace, torch.float32, "c_trace") if c_trace is not None else None, ldt,
+            wp, wb, _stream_ptr(stream)))
+    return Recovered(X, R, n_iter, idx_trace, c_trace, workspace)
 
 
 def _host(t: torch.Tensor, dtype, what: str):

@@ -183,11 +183,12 @@ mp_status mp_recover(const float* psi_t, int N, int M, int64_t ld,
     return launch_recover_streamloop(a, ws, s);
 }
 
-mp_status mp_recover_batched(const float* psi_t, int N, int M, int64_t ld,
-                             const float* Y, int64_t ldy, int B,
-                             float eps, int max_iter,
-                             float* X, float* R, int* n_iter,
-                             void* workspace, size_t workspace_bytes, void* stream)
+mp_status mp_recover_batched_traced(const float* psi_t, int N, int M, int64_t ld,
+                                    const float* Y, int64_t ldy, int B,
+                                    float eps, int max_iter,
+                                    float* X, float* R, int* n_iter,
+                                    int* idx_trace, float* c_trace, int64_t ldt,
+                                    void* workspace, size_t workspace_bytes, void* stream)
 {
     mp_status st = check_dictionary(psi_t, N, M, ld);
     if (st != MP_OK) return st;
@@ -197,13 +198,24 @@ mp_status mp_recover_batched(const float* psi_t, int N, int M, int64_t ld,
     if (ldy < N || (ldy & 3)) return fail(MP_ERR_INVALID_ARG, "need ldy >= N and ldy %% 4 == 0");
     if (max_iter < 0) return fail(MP_ERR_INVALID_ARG, "max_iter must be >= 0 (got %d)", max_iter);
     if (!(eps >= 0.0f)) return fail(MP_ERR_INVALID_ARG, "eps must be >= 0 and not NaN");
+    if ((idx_trace || c_trace) && ldt < max_iter) return fail(MP_ERR_INVALID_ARG, "need ldt >= max_iter");
     const size_t need = mp_workspace_bytes(N, M, B);
     if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 255u) || workspace_bytes < need)
         return fail(MP_ERR_WORKSPACE, "workspace must be non-null, 256-byte aligned and >= %zu bytes (got %zu)", need, workspace_bytes);
     Workspace ws;
     workspace_layout(N, M, B, workspace, &ws);
-    BatchedArgs a{psi_t, N, M, ld, Y, ldy, B, eps, max_iter, X, R, n_iter};
+    BatchedArgs a{psi_t, N, M, ld, Y, ldy, B, eps, max_iter, X, R, n_iter, idx_trace, c_trace, ldt};
     return launch_recover_batched(a, ws, static_cast<cudaStream_t>(stream));
+}
+
+mp_status mp_recover_batched(const float* psi_t, int N, int M, int64_t ld,
+                             const float* Y, int64_t ldy, int B,
+                             float eps, int max_iter,
+                             float* X, float* R, int* n_iter,
+                             void* workspace, size_t workspace_bytes, void* stream)
+{
+    return mp_recover_batched_traced(psi_t, N, M, ld, Y, ldy, B, eps, max_iter, X, R, n_iter, nullptr, nullptr, 0,
+                                     workspace, workspace_bytes, stream);
 }
 
 // ---------------------------------------------------------------------------------------------------------

@@ -12,7 +12,9 @@ static mp_status launch_batched_sequential(const BatchedArgs& a, const Workspace
     workspace_layout(a.N, a.M, 1, ws.ctrl, &one);
     for (int b = 0; b < a.B; b++) {
         RecoverArgs s{a.psi_t, a.N, a.M, a.ld, a.Y + (int64_t)b * a.ldy, a.eps, a.max_iter,
-                      a.X + (int64_t)b * a.M, a.R + (int64_t)b * a.N, a.n_iter + b, nullptr, nullptr};
+                      a.X + (int64_t)b * a.M, a.R + (int64_t)b * a.N, a.n_iter + b,
+                      a.idx_trace ? a.idx_trace + (int64_t)b * a.ldt : nullptr,
+                      a.c_trace ? a.c_trace + (int64_t)b * a.ldt : nullptr};
         mp_status st = (options().algo != 2 && persistent_supported(a.N, a.M))
                            ? launch_recover_persistent(s, one, stream)
                            : launch_recover_streamloop(s, one, stream);

@@ -61,6 +61,7 @@ struct BatchedArgs {
     const float* psi_t; int N, M; int64_t ld;
     const float* Y; int64_t ldy; int B; float eps; int max_iter;
     float* X; float* R; int* n_iter;
+    int* idx_trace; float* c_trace; int64_t ldt;
 };
 mp_status launch_recover_batched(const BatchedArgs& a, const Workspace& ws, cudaStream_t stream);
 

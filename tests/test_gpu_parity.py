@@ -1,0 +1,272 @@
+"""GPU parity tests: the CUDA path (through the C ABI, via the thin binding) against the CPU oracle on the
+same seeded inputs.  Contract and readings: tests/grading.py and DESIGN.md.  Run on a B200: pytest -m gpu.
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_0809_1833_b200 import synth
+import grading
+import problems
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def mp():
+    import paper_0809_1833_b200 as m
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    yield m
+    m.mp_set_int("algo", 0)
+    m.mp_set_int("batched_algo", 0)
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def run_single(mp, psi32, y32, eps, max_iter, algo=0, ld=None):
+    """-> (x, r, n_iter, idx, c) as numpy"""
+    mp.mp_set_int("algo", algo)
+    M, N = psi32.shape
+    if ld is None:
+        ld = (N + 3) // 4 * 4
+    buf = torch.full((M, ld), 7.0, dtype=torch.float32, device="cuda")     # pad columns hold garbage on purpose
+    buf[:, :N] = dev(psi32)
+    psi_d = buf[:, :N]
+    res = mp.mp_recover(psi_d, dev(y32), eps, max_iter, trace=True)
+    torch.cuda.synchronize()
+    t = int(res.n_iter.item())
+    return (res.x.cpu().numpy(), res.r.cpu().numpy(), t, res.idx_trace.cpu().numpy()[:t], res.c_trace.cpu().numpy()[:t])
+
+
+ALGOS = [1, 2]
+
+
+# ------------------------------------------------------------------------------------------ normalisation (a0)
+@pytest.mark.parametrize("N,M", [(256, 1024), (250, 33), (1, 5), (4096, 300), (37, 1000)])
+def test_normalize_columns_matches_float64_quotient(mp, N, M):
+    """Eq. 4: fp32 result == float64 normalise-then-round, to <= 1 ulp; ||psi_m|| = 1 to 2e-7."""
+    raw = synth.gaussian_dictionary(N, M, seed=11)
+    raw[M // 2] = 0.0                                                       # a zero atom stays zero (reading R7)
+    ld = (N + 3) // 4 * 4
+    buf = torch.full((M, ld), 3.0, dtype=torch.float32, device="cuda")
+    buf[:, :N] = dev(raw)
+    norms = torch.empty(M, dtype=torch.float32, device="cuda")
+    mp.mp_normalize_columns(buf[:, :N], norms)
+    torch.cuda.synchronize()
+    got = buf[:, :N].cpu().numpy()
+    ref64, n64 = oracle.normalize_columns(raw)
+    ref = ref64.astype(np.float32)
+    ulp = np.spacing(np.abs(ref)).astype(np.float64)
+    assert np.all(np.abs(got.astype(np.float64) - ref.astype(np.float64)) <= ulp)
+    assert np.array_equal(got, ref) or np.mean(got != ref) < 1e-3           # float64 quotient rounded once: essentially always equal
+    np.testing.assert_allclose(norms.cpu().numpy(), n64, rtol=1e-6)
+    nn = np.linalg.norm(got.astype(np.float64), axis=1)
+    keep = np.arange(M) != M // 2
+    assert np.all(np.abs(nn[keep] - 1.0) <= 2e-7) and nn[M // 2] == 0.0
+    if ld > N:
+        assert torch.all(buf[:, N:] == 3.0)                                  # pad columns untouched
+
+
+def test_normalize_leaves_unit_bernoulli_unchanged(mp):
+    """Eq. 13: +-1/sqrt(N) atoms are unit already; with N a power of 4 the kernel returns them bit-identical."""
+    raw = synth.bernoulli_dictionary(1024, 200, seed=5)
+    d = dev(raw)
+    mp.mp_normalize_columns(d)
+    assert np.array_equal(d.cpu().numpy(), raw)
+
+
+# ------------------------------------------------------------------------------------------ CFG1, all seeds, both algorithms
+@pytest.mark.parametrize("algo", ALGOS)
+@pytest.mark.parametrize("seed", [1, 2, 3])
+def test_cfg1_full_grading(mp, seed, algo):
+    pb = problems.make_problem(synth.config("cfg1"), seed)
+    c = pb.cfg
+    x, r, t, idx, cc = run_single(mp, pb.psi32, pb.Y[0], c.eps, c.max_iter, algo)
+    g = grading.grade_single(pb.psi32, pb.Y[0], c.eps, c.max_iter, x, r, t, idx, cc, x_true=pb.X[0], support=pb.S[0])
+    assert g.exact_recovery
+    assert g.first_divergence >= 0 or g.n_iter_gpu == g.n_iter_ref or abs(g.n_iter_gpu - g.n_iter_ref) == 1
+
+
+# ------------------------------------------------------------------------------------------ ragged shapes / several tiles + tail
+RAGGED = [
+    # N,    M,    K,  ld     what it exercises
+    (250, 1000, 10, None),   # N % 4 != 0 (pad columns in ld), M not a multiple of anything
+    (37, 5, 2, 40),          # fewer atoms than CTAs, tiny N
+    (1, 3, 1, 4),            # N = 1
+    (130, 149, 6, 256),      # ld > Npad (non-contiguous atoms), M = grid + 1
+    (2052, 777, 20, None),   # N just above a 128 multiple
+    (5000, 600, 24, None),   # row > one pipeline slot: column-chunked path
+    (8192, 320, 16, None),   # largest N of the configs
+    (512, 4099, 24, None),   # many atoms per CTA, ragged tail
+]
+
+
+@pytest.mark.parametrize("algo", ALGOS)
+@pytest.mark.parametrize("N,M,K,ld", RAGGED)
+def test_ragged_shapes_full_grading(mp, N, M, K, ld, algo):
+    cfg = problems.custom_config(N, M, K, eps=1e-4, max_iter=6 * K + 3)
+    pb = problems.make_problem(cfg, seed=4)
+    x, r, t, idx, cc = run_single(mp, pb.psi32, pb.Y[0], cfg.eps, cfg.max_iter, algo, ld)
+    grading.grade_single(pb.psi32, pb.Y[0], cfg.eps, cfg.max_iter, x, r, t, idx, cc)
+
+
+# ------------------------------------------------------------------------------------------ edge / degenerate cases
+@pytest.mark.parametrize("algo", ALGOS)
+def test_edge_cases(mp, algo):
+    pb = problems.make_problem(problems.custom_config(64, 200, 4), seed=2)
+    y = pb.Y[0]
+    # y = 0 -> 0 iterations (0 > eps*0 is false)
+    x, r, t, _, _ = run_single(mp, pb.psi32, np.zeros_like(y), 1e-5, 50, algo)
+    assert t == 0 and not x.any() and not r.any()
+    # max_iter = 0 -> x = 0, r = y
+    x, r, t, _, _ = run_single(mp, pb.psi32, y, 1e-5, 0, algo)
+    assert t == 0 and not x.any() and np.array_equal(r, y)
+    # eps >= 1 -> ||y|| > eps ||y|| is false
+    x, r, t, _, _ = run_single(mp, pb.psi32, y, 1.0, 50, algo)
+    assert t == 0 and np.array_equal(r, y)
+    # eps = 0 -> runs to max_iter (no exact zero residual on random data)
+    x, r, t, idx, cc = run_single(mp, pb.psi32, y, 0.0, 40, algo)
+    assert t == 40
+    grading.grade_single(pb.psi32, y, 0.0, 40, x, r, t, idx, cc)
+    # max_iter = 1: one gemv + argmax (Eq. 9, Eq. 16)
+    x, r, t, idx, cc = run_single(mp, pb.psi32, y, 0.0, 1, algo)
+    c_ref = oracle.correlate(pb.psi32, y.astype(np.float64))
+    assert t == 1 and idx[0] == oracle.argmax_abs(c_ref) and abs(cc[0] - c_ref[idx[0]]) <= 1e-6 * np.linalg.norm(y)
+
+
+@pytest.mark.parametrize("algo", ALGOS)
+def test_orthonormal_hadamard_recovers_in_k_steps(mp, algo):
+    """north_star pin on the GPU path: Psi = Hadamard/sqrt(N), N = M = 256 (entries +-1/16 exact): K steps, x~ = x."""
+    n = 256
+    H = np.array([[1.0]])
+    while H.shape[0] < n:
+        H = np.block([[H, H], [H, -H]])
+    psi32 = np.ascontiguousarray((H / 16.0).T.astype(np.float32))
+    x_true = np.zeros(n)
+    S = [3, 77, 200, 129, 255, 0]
+    x_true[S] = [2.0, -1.5, 0.75, 3.25, -0.5, 1.0]                          # exactly representable, distinct magnitudes
+    y = (H / 16.0) @ x_true
+    x, r, t, idx, cc = run_single(mp, psi32, y.astype(np.float32), 1e-6, 100, algo)
+    order = [S[k] for k in np.argsort(-np.abs(x_true[S]), kind="stable")]
+    assert t == len(S) and list(idx) == order
+    np.testing.assert_allclose(x, x_true, atol=1e-6)
+    assert np.linalg.norm(r) <= 1e-6 * np.linalg.norm(y)
+
+
+@pytest.mark.parametrize("algo", ALGOS)
+def test_tie_break_lowest_index(mp, algo):
+    """Eq. 16: duplicated and negated atoms have exactly equal |c|; the smaller index must win,
+    wherever the two copies fall (same warp, different warps, different CTAs)."""
+    pb = problems.make_problem(problems.custom_config(128, 600, 4), seed=9)
+    psi = pb.psi32.copy()
+    y = pb.Y[0]
+    c = oracle.correlate(psi, y.astype(np.float64))
+    best = int(oracle.argmax_abs(c))
+    for other, sign in [(best + 1 if best + 1 < 600 else best - 1, 1.0), (599 - best if 599 - best != best else 0, -1.0), (0 if best else 1, 1.0)]:
+        p = psi.copy()
+        p[other] = sign * p[best]
+        x, r, t, idx, cc = run_single(mp, p, y, 0.0, 1, algo)
+        assert idx[0] == min(best, other), (best, other, idx[0])
+        assert np.sign(cc[0]) == (np.sign(c[best]) if idx[0] == best else sign * np.sign(c[best]))
+    # all |c| equal: Hadamard/sqrt(N) with y = e_0 -> index 0
+    n = 64
+    H = np.array([[1.0]])
+    while H.shape[0] < n:
+        H = np.block([[H, H], [H, -H]])
+    e0 = np.zeros(n, np.float32); e0[0] = 1.0
+    x, r, t, idx, cc = run_single(mp, np.ascontiguousarray((H / 8.0).T.astype(np.float32)), e0, 0.0, 1, algo)
+    assert idx[0] == 0 and cc[0] == 0.125
+
+
+def test_rerun_is_bit_identical_and_workspace_reusable(mp):
+    """Deterministic reduction order: two runs give identical bits; a dirty workspace does not matter."""
+    pb = problems.make_problem(synth.config("cfg1"), 2)
+    mp.mp_set_int("algo", 0)
+    psi_d, y_d = dev(pb.psi32), dev(pb.Y[0])
+    ws = torch.empty(mp.mp_workspace_bytes(256, 1024, 1) + 256, dtype=torch.uint8, device="cuda").fill_(0xAB)
+    a = mp.mp_recover(psi_d, y_d, 1e-5, 4096, trace=True, workspace=ws)
+    torch.cuda.synchronize()
+    xa, ra, ta = a.x.clone(), a.r.clone(), int(a.n_iter.item())
+    ia = a.idx_trace[:ta].clone()
+    b = mp.mp_recover(psi_d, y_d, 1e-5, 4096, trace=True, workspace=ws)
+    torch.cuda.synchronize()
+    assert int(b.n_iter.item()) == ta and torch.equal(b.x, xa) and torch.equal(b.r, ra) and torch.equal(b.idx_trace[:ta], ia)
+
+
+def test_invalid_arguments_on_device(mp):
+    pb = problems.make_problem(problems.custom_config(64, 100, 3), seed=1)
+    psi_d, y_d = dev(pb.psi32), dev(pb.Y[0])
+    with pytest.raises(mp.MPError) as e:
+        mp.mp_recover(psi_d, y_d, -1.0, 10)
+    assert e.value.status == mp.MP_ERR_INVALID_ARG
+    with pytest.raises(mp.MPError) as e:
+        mp.mp_recover(psi_d, y_d, 1e-5, 10, workspace=torch.empty(300, dtype=torch.uint8, device="cuda"))
+    assert e.value.status == mp.MP_ERR_WORKSPACE
+
+
+# ------------------------------------------------------------------------------------------ CFG2 (full replay) and CFG3 (sampled)
+def test_cfg2_full_grading(mp):
+    pb = problems.make_problem(synth.config("cfg2"), 1)
+    c = pb.cfg
+    x, r, t, idx, cc = run_single(mp, pb.psi32, pb.Y[0], c.eps, c.max_iter, 0)
+    g = grading.grade_single(pb.psi32, pb.Y[0], c.eps, c.max_iter, x, r, t, idx, cc, x_true=pb.X[0], support=pb.S[0])
+    assert g.exact_recovery and 500 < g.n_iter_gpu < 1200
+
+
+def test_cfg3_full_size_sampled_grading(mp):
+    """BASELINE.json's headline size (N=4096, M=16384, 256 MiB Psi) in the launch configuration bench.py times:
+    every 97th iteration plus the first/last few are rebuilt in float64 from the GPU trace and checked one by one;
+    properties that hold at any size (monotone norm via the trace, stop rule, support) are checked on all."""
+    pb = problems.make_problem(synth.config("cfg3"), 1)
+    c = pb.cfg
+    x, r, t, idx, cc = run_single(mp, pb.psi32, pb.Y[0], c.eps, c.max_iter, 0)
+    assert 800 < t < 2500
+    ts = sorted(set(list(range(0, 4)) + list(range(5, t, 97)) + list(range(t - 3, t))))
+    grading.grade_sampled(pb.psi32, pb.Y[0], idx, cc, t, r, ts)
+    # support: MP at N = 16K never picks an off-support atom -> selected atoms == true support
+    assert set(idx.tolist()) == set(pb.S[0].tolist())
+    coef = np.zeros(c.M); np.add.at(coef, idx, cc.astype(np.float64))
+    assert np.all(np.abs(x - coef) <= 6e-8 * np.abs(coef) + 1e-45)
+    assert np.linalg.norm(x - pb.X[0]) <= 1e-4 * np.linalg.norm(pb.X[0])
+    ny = np.linalg.norm(pb.Y[0].astype(np.float64))
+    assert np.linalg.norm(r.astype(np.float64)) <= np.float32(c.eps) * ny * (1 + 1e-6)
+
+
+# ------------------------------------------------------------------------------------------ batched (a9)
+@pytest.mark.parametrize("B,N,M,K", [(3, 256, 1024, 16), (5, 250, 333, 8), (64, 128, 512, 6)])
+def test_batched_every_signal_graded_like_a_single_run(mp, B, N, M, K):
+    """P:165 / reading R17: signal b's result is MP on (Psi, y_b) under the same rules as the single-signal path
+    (full teacher-forced grading per signal through the traced entry point); finished signals are frozen."""
+    cfg = problems.custom_config(N, M, K, eps=1e-5, max_iter=10 * K, B=B)
+    pb = problems.make_problem(cfg, seed=6)
+    pb.Y[B // 2] = 0.0                                                       # one signal that stops at once
+    ld = (N + 3) // 4 * 4
+    buf = torch.full((M, ld), 5.0, dtype=torch.float32, device="cuda"); buf[:, :N] = dev(pb.psi32)
+    Yb = torch.full((B, ld), 9.0, dtype=torch.float32, device="cuda"); Yb[:, :N] = dev(pb.Y)
+    res = mp.mp_recover_batched(buf[:, :N], Yb[:, :N], cfg.eps, cfg.max_iter, trace=True)
+    torch.cuda.synchronize()
+    X, R, T = res.x.cpu().numpy(), res.r.cpu().numpy(), res.n_iter.cpu().numpy()
+    I, Cc = res.idx_trace.cpu().numpy(), res.c_trace.cpu().numpy()
+    assert T[B // 2] == 0 and not X[B // 2].any() and not R[B // 2].any()
+    for b in range(B):
+        t = int(T[b])
+        grading.grade_single(pb.psi32, pb.Y[b], cfg.eps, cfg.max_iter, X[b], R[b], t, I[b, :t], Cc[b, :t],
+                             x_true=pb.X[b], support=pb.S[b], nthreads=1)
+    # and the untraced entry point gives the same bits
+    res2 = mp.mp_recover_batched(buf[:, :N], Yb[:, :N], cfg.eps, cfg.max_iter)
+    torch.cuda.synchronize()
+    assert torch.equal(res2.x, res.x) and torch.equal(res2.r, res.r) and torch.equal(res2.n_iter, res.n_iter)
+
+
+# ------------------------------------------------------------------------------------------ host-buffer entry points (e2e path)
+def test_host_entry_point_matches_device_entry_point(mp):
+    pb = problems.make_problem(synth.config("cfg1"), 3)
+    mp.mp_set_int("algo", 0)
+    h = mp.mp_recover_host(torch.from_numpy(pb.psi_raw), torch.from_numpy(pb.Y[0]), 1e-5, 4096, normalize=True, trace=True)
+    t = int(h.n_iter.item())
+    x, r, t2, idx, cc = run_single(mp, pb.psi32, pb.Y[0], 1e-5, 4096, 0)
+    assert t == t2 and np.array_equal(h.idx_trace.numpy()[:t], idx)
+    assert np.array_equal(h.x.numpy(), x) and np.array_equal(h.r.numpy(), r)
