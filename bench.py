@@ -140,6 +140,18 @@ def run_reference(args, cfg):
         "gpu_launches": 0}))
 
 
+def aggregate(dist, elapsed_local, units_local, device):
+    """Whole-job figures of a replicas-only run: the elapsed time is the MAX over ranks, the
+    units (MP iterations) are the SUM over ranks.  `dist` is torch.distributed or None (single process)."""
+    import torch
+    t = torch.tensor([float(elapsed_local)], dtype=torch.float64, device=device)
+    u = torch.tensor([float(units_local)], dtype=torch.float64, device=device)
+    if dist is not None and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
 def workload_name(cfg):
     return (f"{cfg.name}: single-signal MP fp32, N={cfg.N}, M={cfg.M}, K={cfg.K}, {cfg.dictionary} dictionary, "
             f"eps={cfg.eps:g}, max_iter={cfg.max_iter}" + (f", B={cfg.B}" if cfg.B > 1 else ""))
@@ -242,13 +254,8 @@ def main():
     ms_solve = [ev[2 + 2 * k].elapsed_time(ev[3 + 2 * k]) for k in range(args.steps)]
     its_per_step = int(n_d.sum().item())
     its_max = int(n_d.max().item())
-    t_all = torch.tensor([ms_total], dtype=torch.float64, device=dev)
-    its_all = torch.tensor([float(its_per_step * args.steps)], dtype=torch.float64, device=dev)
-    if dist:
-        dist.all_reduce(t_all, op=dist.ReduceOp.MAX)
-        dist.all_reduce(its_all, op=dist.ReduceOp.SUM)
-    ms_total_max = float(t_all.item())
-    value = float(its_all.item()) / (ms_total_max * 1e-3)
+    ms_total_max, its_sum = aggregate(dist, ms_total, float(its_per_step * args.steps), dev)
+    value = its_sum / (ms_total_max * 1e-3)
 
     # ---- roofline of the dominant kernel (the persistent MP loop; one launch per solve) -------------------------
     peak, peak_src = load_peaks()
@@ -274,12 +281,10 @@ def main():
         for _ in range(args.steps):
             its += int(mp.mp_recover_host(hp, hy, cfg.eps, cfg.max_iter, normalize=True, device=local).n_iter.item())
         dt = time.perf_counter() - t0
-        t_e = torch.tensor([dt], dtype=torch.float64, device=dev); i_e = torch.tensor([float(its)], dtype=torch.float64, device=dev)
-        if dist:
-            dist.all_reduce(t_e, op=dist.ReduceOp.MAX); dist.all_reduce(i_e, op=dist.ReduceOp.SUM)
-        e2e = {"value": float(i_e.item()) / float(t_e.item()), "unit": UNIT,
+        dt_max, its_e = aggregate(dist, dt, float(its), dev)
+        e2e = {"value": its_e / dt_max, "unit": UNIT,
                "h2d_bytes_per_step": 4 * N * M + 4 * N, "d2h_bytes_per_step": 4 * M + 4 * N + 4,
-               "ms_per_step": 1e3 * float(t_e.item()) / args.steps,
+               "ms_per_step": 1e3 * dt_max / args.steps,
                "note": "mp_recover_host: cudaMalloc + H2D(Psi, y) + normalise + solve + D2H(x, r, n_iter) + free per step"}
 
     if rank == 0:

@@ -1,0 +1,74 @@
+"""Host-side logic of bench.py on CPU: replicas-only aggregation under world_size-2 gloo,
+the reference arm's rank handling, and the JSON contract of the `--impl reference` line."""
+import json
+import os
+import socket
+import subprocess
+import sys
+
+import pytest
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as tmp
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+sys.path.insert(0, ROOT)
+
+
+def _free_port():
+    s = socket.socket(); s.bind(("127.0.0.1", 0)); p = s.getsockname()[1]; s.close()
+    return p
+
+
+def _worker(rank, world, port, out):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    import bench
+    # rank r took (10 + 5 r) ms for (1000 + 100 r) iterations
+    t, u = bench.aggregate(dist, 10.0 + 5.0 * rank, 1000.0 + 100.0 * rank, torch.device("cpu"))
+    out.put((rank, t, u))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_aggregate_world2_gloo():
+    ctx = tmp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs: p.start()
+    got = sorted(q.get(timeout=120) for _ in range(2))
+    for p in procs:
+        p.join(60); assert p.exitcode == 0
+    for rank, t, u in got:
+        assert t == 15.0          # max over ranks
+        assert u == 2100.0        # sum over ranks: whole-job units
+    # whole-job value = sum(units) / max(time)
+    assert got[0][2] / (got[0][1] * 1e-3) == pytest.approx(140000.0)
+
+
+def test_aggregate_single_process():
+    import bench
+    assert bench.aggregate(None, 3.5, 7.0, torch.device("cpu")) == (3.5, 7.0)
+
+
+def _run_reference(rank, world):
+    env = dict(os.environ, RANK=str(rank), WORLD_SIZE=str(world), LOCAL_RANK=str(rank))
+    return subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--config", "cfg1",
+                           "--gpus", str(world), "--steps", "1", "--warmup", "0"], env=env, capture_output=True,
+                          text=True, timeout=300)
+
+
+def test_reference_arm_rank0_prints_contract_line():
+    p = _run_reference(0, 2)
+    assert p.returncode == 0, p.stderr
+    line = json.loads(p.stdout.strip().splitlines()[-1])
+    assert line["impl"] == "reference" and line["metric"] == "mp_iterations_per_s" and line["higher_is_better"]
+    assert line["value"] > 0 and line["cpu_baseline"]["kind"] == "oracle" and line["cpu_baseline"]["value"] == line["value"]
+    assert line["e2e"]["value"] == line["value"] and line["e2e"]["h2d_bytes_per_step"] == 0
+    assert line["gpu_launches"] == 0 and line["vs_baseline"] is None and "workload" in line["config"]
+
+
+def test_reference_arm_other_ranks_exit_silently():
+    p = _run_reference(1, 2)
+    assert p.returncode == 0 and p.stdout.strip() == ""
