@@ -108,6 +108,17 @@ MP_API mp_status mp_recover_batched_traced(const float* psi_t, int N, int M, int
                                     int* idx_trace, float* c_trace, int64_t ldt,
                                     void* workspace, size_t workspace_bytes, void* stream);
 
+/* The correlation step of the batched path alone (Eq. 9 / Eq. 15 for B signals at once, NS subsystem 5):
+ *   C[b*M + m] = <Y[b], psi_m>,   b < B <= 64,   C out B x M row-major (device).
+ * Runs the same split-TF32 tensor-core contraction (tcgen05, TMEM accumulators, split-K over a 4-CTA cluster)
+ * that mp_recover_batched runs every iteration, so the contraction can be checked element by element.
+ * Needs mp_correlate_batched_workspace_bytes(N, M, B) bytes of 256-byte aligned workspace.
+ * MP_ERR_UNSUPPORTED if the shape does not fit the tensor-core kernel (N <= 96). */
+MP_API size_t mp_correlate_batched_workspace_bytes(int N, int M, int B);
+MP_API mp_status mp_correlate_batched(const float* psi_t, int N, int M, int64_t ld,
+                               const float* Y, int64_t ldy, int B, float* C,
+                               void* workspace, size_t workspace_bytes, void* stream);
+
 /* Description of the last error on this thread ("" if none).  Static storage, never NULL. */
 MP_API const char* mp_last_error(void);
 
@@ -117,7 +128,9 @@ MP_API const char* mp_last_error(void);
  *   "warps"         consumer warps per CTA of the persistent kernel (0 = auto)
  *   "slot_bytes"    bytes of one shared-memory stage (0 = auto);   "depth"  stages per warp (0 = auto)
  *   "grid"          CTAs of the persistent kernel (0 = auto = one per SM)
- *   "chunk"         iterations enqueued between stop-flag polls of algo 2 (default 64) */
+ *   "chunk"         iterations enqueued between stop-flag polls of algo 2 (default 64)
+ *   "batched_algo"  0 = auto (default): lock-step tensor-core kernel in groups of <= 64 signals when the shape fits,
+ *                   1 = tensor-core kernel or MP_ERR_UNSUPPORTED, 2 = one single-signal solve after another */
 MP_API mp_status mp_set_int(const char* name, int64_t value);
 MP_API mp_status mp_get_int(const char* name, int64_t* value);
 

@@ -50,6 +50,10 @@ lib.mp_recover_batched.restype = _i
 lib.mp_recover_batched.argtypes = [_vp, _i, _i, _i64, _vp, _i64, _i, _f, _i, _vp, _vp, _vp, _vp, _sz, _vp]
 lib.mp_recover_batched_traced.restype = _i
 lib.mp_recover_batched_traced.argtypes = [_vp, _i, _i, _i64, _vp, _i64, _i, _f, _i, _vp, _vp, _vp, _vp, _vp, _i64, _vp, _sz, _vp]
+lib.mp_correlate_batched_workspace_bytes.restype = _sz
+lib.mp_correlate_batched_workspace_bytes.argtypes = [_i, _i, _i]
+lib.mp_correlate_batched.restype = _i
+lib.mp_correlate_batched.argtypes = [_vp, _i, _i, _i64, _vp, _i64, _i, _vp, _vp, _sz, _vp]
 lib.mp_last_error.restype = C.c_char_p
 lib.mp_last_error.argtypes = []
 lib.mp_set_int.restype = _i
@@ -191,6 +195,26 @@ def mp_recover_batched(psi_t: torch.Tensor, Y: torch.Tensor, eps: float, max_ite
             _dev(c_trace, torch.float32, "c_trace") if c_trace is not None else None, ldt,
             wp, wb, _stream_ptr(stream)))
     return Recovered(X, R, n_iter, idx_trace, c_trace, workspace)
+
+
+def mp_correlate_batched(psi_t: torch.Tensor, Y: torch.Tensor, *, C_out=None, stream=None) -> torch.Tensor:
+    """C[b, m] = <Y[b], psi_m> by the tensor-core contraction of the batched path (Eq. 9 for B <= 64 signals)."""
+    p, N, M, ld = _dict_args(psi_t)
+    dev = psi_t.device
+    if not (Y.is_cuda and Y.dtype == torch.float32 and Y.dim() == 2 and Y.shape[1] == N and (N == 1 or Y.stride(1) == 1)):
+        raise TypeError("Y must be a CUDA float32 [B, N] tensor with unit stride along N")
+    B = Y.shape[0]
+    ldy = Y.stride(0) if B > 1 else max(Y.stride(0), N)
+    C_out = torch.empty(B, M, dtype=torch.float32, device=dev) if C_out is None else C_out
+    need = lib.mp_correlate_batched_workspace_bytes(N, M, B)
+    ws = torch.empty(need + 256, dtype=torch.uint8, device=dev)
+    base = ws.data_ptr()
+    off = (-base) % 256
+    with torch.cuda.device(dev):
+        _check(lib.mp_correlate_batched(p, N, M, ld, Y.data_ptr(), ldy, B, _dev(C_out, torch.float32, "C"),
+                                        base + off, ws.numel() - off, _stream_ptr(stream)))
+    C_out._mp_workspace = ws          # keep the workspace alive until the stream has run the kernel
+    return C_out
 
 
 def _host(t: torch.Tensor, dtype, what: str):

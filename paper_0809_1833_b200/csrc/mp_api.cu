@@ -64,8 +64,9 @@ size_t workspace_layout(int N, int M, int B, void* base, Workspace* ws)
     const size_t o_x64 = take(sizeof(double) * (size_t)B * M);     // must directly follow ctrl (one memset covers both)
     const size_t o_r64 = take(sizeof(double) * (size_t)B * Nr);
     const size_t o_r32 = take(sizeof(float) * (size_t)B * Nr);
-    const size_t o_keys = take(sizeof(unsigned long long) * 3 * (size_t)B);
+    const size_t o_keys = take(sizeof(unsigned long long) * 3 * (size_t)(B > 1 && B < 64 ? 64 : B));
     const size_t o_state = take(sizeof(int) * 4 * (size_t)B);
+    const size_t o_rs = B > 1 ? take(sizeof(float) * 128 * Nr) : off;
     if (ws) {
         ws->ctrl = reinterpret_cast<unsigned long long*>(b + o_ctrl);
         ws->x64 = reinterpret_cast<double*>(b + o_x64);
@@ -73,6 +74,7 @@ size_t workspace_layout(int N, int M, int B, void* base, Workspace* ws)
         ws->r32 = reinterpret_cast<float*>(b + o_r32);
         ws->keys = reinterpret_cast<unsigned long long*>(b + o_keys);
         ws->state = reinterpret_cast<int*>(b + o_state);
+        ws->rs = B > 1 ? reinterpret_cast<float*>(b + o_rs) : nullptr;
         ws->bytes = off;
     }
     return off;
@@ -216,6 +218,40 @@ mp_status mp_recover_batched(const float* psi_t, int N, int M, int64_t ld,
 {
     return mp_recover_batched_traced(psi_t, N, M, ld, Y, ldy, B, eps, max_iter, X, R, n_iter, nullptr, nullptr, 0,
                                      workspace, workspace_bytes, stream);
+}
+
+mp_status mp_correlate_batched(const float* psi_t, int N, int M, int64_t ld,
+                               const float* Y, int64_t ldy, int B, float* C,
+                               void* workspace, size_t workspace_bytes, void* stream)
+{
+    mp_status st = check_dictionary(psi_t, N, M, ld);
+    if (st != MP_OK) return st;
+    if (B < 1 || B > 64) return fail(MP_ERR_INVALID_ARG, "need 1 <= B <= 64 (got %d)", B);
+    if (!Y || !C) return fail(MP_ERR_INVALID_ARG, "Y and C must be non-null");
+    if (!aligned16(Y) || !aligned16(C)) return fail(MP_ERR_INVALID_ARG, "Y and C must be 16-byte aligned");
+    if (ldy < N || (ldy & 3)) return fail(MP_ERR_INVALID_ARG, "need ldy >= N and ldy %% 4 == 0");
+    const int Bw = B < 2 ? 2 : B;                                   // the batched workspace layout (B > 1)
+    const size_t scratch_off = (mp_workspace_bytes(N, M, Bw) + 255) / 256 * 256;
+    const size_t need = scratch_off + sizeof(float) * ((size_t)Bw * M + (size_t)Bw * N) + sizeof(int) * (size_t)Bw + 512;
+    if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 255u) || workspace_bytes < need)
+        return fail(MP_ERR_WORKSPACE, "workspace must be non-null, 256-byte aligned and >= %zu bytes (got %zu)", need, workspace_bytes);
+    Workspace ws;
+    workspace_layout(N, M, Bw, workspace, &ws);
+    // scratch X, R, n_iter of the one iteration that is run
+    char* sc = static_cast<char*>(workspace) + scratch_off;
+    float* X = reinterpret_cast<float*>(sc);
+    float* R = X + (size_t)Bw * M;
+    int* n_iter = reinterpret_cast<int*>(R + (size_t)Bw * N);
+    BatchedArgs a{psi_t, N, M, ld, Y, ldy, B, 0.0f, 1, X, R, n_iter, nullptr, nullptr, 0};
+    return launch_recover_batched_tc(a, ws, C, static_cast<cudaStream_t>(stream));
+}
+
+size_t mp_correlate_batched_workspace_bytes(int N, int M, int B)
+{
+    if (N < 1 || M < 1 || B < 1 || B > 64) return 0;
+    const int Bw = B < 2 ? 2 : B;
+    const size_t scratch_off = (mp_workspace_bytes(N, M, Bw) + 255) / 256 * 256;
+    return scratch_off + sizeof(float) * ((size_t)Bw * M + (size_t)Bw * N) + sizeof(int) * (size_t)Bw + 512;
 }
 
 // ---------------------------------------------------------------------------------------------------------

@@ -1,5 +1,6 @@
 // mp_batched.cu -- B signals sharing one dictionary.
-// batched_algo 2: one single-signal solve after another on the stream (baseline for the fused path).
+// Dispatch of the batched path, and batched_algo 2: one single-signal solve after another on the stream
+// (the FP32-CUDA-core baseline of the tensor-core kernel in mp_batched_tc.cu).
 #include "mp_common.cuh"
 #include "mp_internal.h"
 
@@ -23,9 +24,27 @@ static mp_status launch_batched_sequential(const BatchedArgs& a, const Workspace
     return MP_OK;
 }
 
+// batched_algo 0 = auto: the lock-step tensor-core kernel (mp_batched_tc.cu) in groups of at most 64 signals when the
+// shape fits it, else the sequential baseline.  1 = tensor-core kernel or error.  2 = sequential.
 mp_status launch_recover_batched(const BatchedArgs& a, const Workspace& ws, cudaStream_t stream)
 {
-    return launch_batched_sequential(a, ws, stream);
+    const int64_t algo = options().batched_algo;
+    if (algo == 2) return launch_batched_sequential(a, ws, stream);
+    const int group = a.B < 64 ? a.B : 64;
+    if (algo == 0 && !batched_tc_supported(a.N, a.M, group)) return launch_batched_sequential(a, ws, stream);
+    for (int b0 = 0; b0 < a.B; b0 += 64) {
+        BatchedArgs g = a;
+        g.B = a.B - b0 < 64 ? a.B - b0 : 64;
+        g.Y = a.Y + (int64_t)b0 * a.ldy;
+        g.X = a.X + (int64_t)b0 * a.M;
+        g.R = a.R + (int64_t)b0 * a.N;
+        g.n_iter = a.n_iter + b0;
+        g.idx_trace = a.idx_trace ? a.idx_trace + (int64_t)b0 * a.ldt : nullptr;
+        g.c_trace = a.c_trace ? a.c_trace + (int64_t)b0 * a.ldt : nullptr;
+        mp_status st = launch_recover_batched_tc(g, ws, nullptr, stream);   // groups reuse the workspace in stream order
+        if (st != MP_OK) return st;
+    }
+    return MP_OK;
 }
 
 }  // namespace mp

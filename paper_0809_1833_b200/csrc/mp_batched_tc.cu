@@ -1,0 +1,576 @@
+// mp_batched_tc.cu -- batched MP: B <= 64 signals share one dictionary and advance in
+// lock-step inside ONE persistent kernel; the correlation step C = Psi^T R (Eq. 9 for every signal at once) is a
+// dense contraction and runs on the 5th-generation tensor cores (tcgen05.mma kind::tf32, accumulators in TMEM)
+// with split-TF32 error compensation so that it holds the fp32 tolerance of DESIGN.md section 4.
+//
+//   * grid = clusters of 4 CTAs, all co-resident.  A cluster owns tiles of AT <= 256 consecutive atoms; inside the
+//     cluster the reduction dimension N is split four ways (split-K), CTA rank q takes k-chunks [q nc/4, (q+1) nc/4).
+//   * per k-chunk of 32 floats one pipeline stage holds the dictionary tile (AT x 32, TMA, 128-byte swizzle, K-major)
+//     and the residual tile (128 x 32: rows 0-63 = tf32-exact high parts of the 64 residuals, rows 64-127 = the
+//     low parts r - hi).  Worker warps derive the low part of the dictionary tile (psi - tf32(psi), exact) into a
+//     second buffer.  The MMA warp then issues, per 8 floats of k,
+//         D_hi[128 x AT] += [R_hi; R_lo] . Psi_hi^T     and     D_lo[128 x AT] += [R_hi; R_lo] . Psi_lo^T
+//     so rows b and 64+b of the two accumulators together hold all four partial products of
+//     (R_hi + R_lo)(Psi_hi + Psi_lo): an UMMA with M = 64 costs the same tensor time as M = 128, so the low-part rows
+//     ride along for free.  The tensor core truncates its fp32 accumulator on every accumulation (measured: a
+//     coherent sum loses about 2^-24.2 relative per UMMA), so the small Psi_lo products get their own accumulator
+//     instead of costing the large one a second truncation per k-step; split-K keeps each chain N/32 UMMAs long.
+//   * epilogue: TMEM -> registers, rows b and 64+b added, the four split-K partials are exchanged through
+//     distributed shared memory and added in rank order (deterministic), CTA q takes a quarter of the tile's atoms,
+//     per-signal packed (|c|, index, sign) argmax (Eq. 16, lowest index on ties) -> red.max.u64 -> grid barrier.
+//   * signal b is owned by CTA b: it applies r_b <- r_b - c psi_i (Eq. 11) to the float64 residual, recomputes
+//     ||r_b||^2 as a direct float64 sum (Eq. 18), x~_b[i] += c (Eq. 10), evaluates the per-signal stop test
+//     and republishes the hi / lo split of the fp32 rounding of r_b for the next contraction; a second grid
+//     barrier hands the new residuals to everybody.  A stopped signal is frozen (reading R17).
+//   * the dictionary never changes, so its TMA loads for iteration t+1 are issued before the barriers of iteration t.
+#include <cuda.h>
+
+#include "mp_internal.h"
+#include "mp_tc.cuh"
+
+namespace mp {
+
+constexpr int kTcThreads = 320;          // warp 0: TMA producer, warp 1: MMA issuer, warps 2-9: split + epilogue workers
+constexpr int kTcWorkers = 256;
+constexpr int kTcCluster = 4;            // split-K ways
+constexpr int kTcMaxStages = 8;
+constexpr int kTcRsTileBytes = 128 * 128;
+constexpr uint32_t kTcTmemCols = 512;    // two accumulators: columns [0, AT) dictionary-hi products, [256, 256 + AT) dictionary-lo products
+
+struct SigState {
+    double thresh;                       // eps * ||y_b||
+    int active, pad;
+};
+
+struct BatchedTcParams {
+    const float* psi_t; int64_t ld;
+    const float* Y; int64_t ldy;
+    float* X; float* R; int* n_iter; int* idx_trace; float* c_trace; int64_t ldt;
+    double* x64; double* r64; float* rs;            // rs: [128][Nr]  rows 0-63 hi parts, rows 64-127 lo parts
+    unsigned long long* ctrl;                       // [0] grid-barrier counter, [5] number of active signals
+    unsigned long long* keys;                       // [3][64] rotating per-signal argmax keys
+    SigState* state;
+    float* dbg_C;                                   // nullable: B x M correlations of iteration 0 (mp_correlate_batched)
+    int N, M, B, Nr, Npad;
+    int AT, n_tiles, n_clusters, tiles_per_cluster, nchunks, S;
+    float eps; int max_iter;
+};
+
+struct TcTail {
+    uint64_t full[kTcMaxStages], empty[kTcMaxStages], lo_full[2], lo_empty[2], tmem_full, tmem_empty, cl_ready, cl_done;
+    unsigned long long skeys[4 * 64];
+    double red[16];
+    uint32_t tmem_base;
+    int n_active;
+};
+
+__device__ __forceinline__ void tc_grid_barrier(unsigned long long* counter, unsigned long long target)
+{
+    fence_proxy_async_all();            // this thread's global writes (residual rows) are later read by TMA in other CTAs
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        red_add_release_u64(counter, 1ull);
+        while (ld_acquire_u64(counter) < target) {}
+        __threadfence();
+    }
+    __syncthreads();
+    fence_proxy_async_all();            // residual rows written by other CTAs are read by TMA (async proxy) next
+}
+
+// Split-TF32 operands.  kind::tf32 reads fp32 words and uses their top 19 bits (sign, exponent, 10 mantissa bits).
+//   dictionary: hi = the raw word as the tensor core sees it (low 13 bits ignored), lo = rn_tf32(psi - trunc(psi));
+//   residual:   hi = rn_tf32(r), lo = rn_tf32(r - hi).
+// The low parts are rounded to nearest HERE, so the hardware conversion of them is exact and the remaining
+// representation error (<= 2^-22 |psi|, <= 2^-23 |r|) has no systematic sign: it averages out over the dot product
+// instead of biasing every correlation the same way, which a truncated low part would.
+__device__ __forceinline__ float tf32_trunc(float v) { return __uint_as_float(__float_as_uint(v) & 0xFFFFE000u); }
+__device__ __forceinline__ float tf32_rn(float v)
+{
+    uint32_t o;
+    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(o) : "f"(v));
+    return __uint_as_float(o);
+}
+
+// block-wide float64 sum in a fixed order (all threads of the CTA call; result uniform)
+__device__ __forceinline__ double tc_block_sum(double v, double* red)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    v = warp_sum(v);
+    __syncthreads();
+    if (lane == 0) red[warp] = v;
+    __syncthreads();
+    double s = 0.0;
+#pragma unroll
+    for (int w = 0; w < kTcThreads / 32; w++) s += red[w];
+    return s;
+}
+
+// writes r (float64) and the hi / lo split of its fp32 rounding
+__device__ __forceinline__ void tc_publish(const BatchedTcParams& p, int b, int n, double v)
+{
+    const float f = (float)v;
+    const float hi = tf32_rn(f);
+    p.r64[(size_t)b * p.Nr + n] = v;
+    p.rs[(size_t)b * p.Nr + n] = hi;
+    p.rs[(size_t)(64 + b) * p.Nr + n] = tf32_rn(f - hi);
+}
+
+__global__ void __launch_bounds__(kTcThreads, 1)
+mp_batched_tc_kernel(const __grid_constant__ CUtensorMap tm_psi, const __grid_constant__ CUtensorMap tm_rs,
+                     const BatchedTcParams p)
+{
+    extern __shared__ unsigned char smem_dyn[];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint32_t q = cluster_ctarank();
+    const int cl = blockIdx.x / kTcCluster;
+    const int G = gridDim.x;
+
+    // ---- shared memory carve-up (1024-byte aligned for the 128-byte swizzle) --------------------------------------
+    const uint32_t base_u32 = (smem_u32(smem_dyn) + 1023u) & ~1023u;
+    unsigned char* base = smem_dyn + (base_u32 - smem_u32(smem_dyn));
+    const int psi_tile_bytes = p.AT * 128;
+    const int stage_bytes = psi_tile_bytes + kTcRsTileBytes;
+    unsigned char* lo_ring = base + (size_t)p.S * stage_bytes;                // 2 x psi_tile_bytes; the epilogue reuses it as P
+    TcTail* tail = reinterpret_cast<TcTail*>(lo_ring + 2 * (size_t)psi_tile_bytes);
+    float* P = reinterpret_cast<float*>(lo_ring);                              // P[col * 64 + b], AT x 64 floats
+
+    if (tid == 0) {
+        for (int s = 0; s < p.S; s++) { mbar_init(&tail->full[s], 2); mbar_init(&tail->empty[s], 1); }
+        for (int j = 0; j < 2; j++) { mbar_init(&tail->lo_full[j], kTcWorkers / 32); mbar_init(&tail->lo_empty[j], 1); }
+        mbar_init(&tail->tmem_full, 1);
+        mbar_init(&tail->tmem_empty, kTcWorkers / 32);
+        mbar_init(&tail->cl_ready, kTcCluster);
+        mbar_init(&tail->cl_done, kTcCluster);
+        mbar_fence_init();
+        prefetch_tensormap(&tm_psi);
+        prefetch_tensormap(&tm_rs);
+    }
+    if (warp == 1) tmem_alloc(&tail->tmem_base, kTcTmemCols);
+    tc_fence_before_sync();
+    __syncthreads();
+    cluster_sync_all();                                                        // peers' mbarriers are initialised
+    tc_fence_after_sync();
+    const uint32_t tmem = tail->tmem_base;
+
+    // ---- this CTA's share of the contraction -----------------------------------------------------------------------
+    const int kc0 = (int)(((int64_t)q * p.nchunks) / kTcCluster);
+    const int kc1 = (int)(((int64_t)(q + 1) * p.nchunks) / kTcCluster);
+    const int my_nc = kc1 - kc0;                                               // >= 1 (host guarantees nchunks >= 4)
+    int n_my_tiles = 0;
+    for (int j = 0; j < p.tiles_per_cluster; j++) n_my_tiles += (cl + j * p.n_clusters) < p.n_tiles ? 1 : 0;
+    const int items = n_my_tiles * my_nc;                                      // pipeline items per MP iteration
+    const uint32_t idesc = umma_idesc_tf32(128, p.AT);
+
+    // ---- Eq. 8 for every signal: r_b <- y_b, ||y_b||, per-signal stop state ------------------------------------------
+    for (int b = blockIdx.x; b < p.B; b += G) {
+        double ss = 0.0;
+        for (int n = tid; n < p.Nr; n += kTcThreads) {
+            const double v = n < p.N ? (double)p.Y[(size_t)b * p.ldy + n] : 0.0;
+            tc_publish(p, b, n, v);
+            ss += v * v;
+        }
+        const double yy = tc_block_sum(ss, tail->red);
+        const double thresh = (double)p.eps * sqrt(yy);
+        const bool active = (sqrt(yy) > thresh) && p.max_iter > 0;
+        if (!active) {
+            for (int n = tid; n < p.N; n += kTcThreads) p.R[(size_t)b * p.N + n] = p.Y[(size_t)b * p.ldy + n];
+        }
+        if (tid == 0) {
+            p.state[b].thresh = thresh;
+            p.state[b].active = active ? 1 : 0;
+            if (active) atomicAdd(p.ctrl + 5, 1ull); else p.n_iter[b] = 0;
+        }
+    }
+    unsigned long long episode = 0;
+    tc_grid_barrier(p.ctrl, ++episode * (unsigned long long)G);
+    if (tid == 0) tail->n_active = (int)ld_acquire_u64(p.ctrl + 5);
+    __syncthreads();
+    int n_active = tail->n_active;
+
+    long long pi = 0, ri = 0;            // producer: dictionary tiles / residual tiles issued so far (running item counts)
+    long long g_mma = 0, g_wrk = 0;      // MMA warp / workers: items consumed so far
+    unsigned int tile_count = 0;         // tiles finished so far (phase of tmem_full / tmem_empty / cl_ready / cl_done)
+    int t = 0;
+
+    while (n_active > 0 && t < p.max_iter) {
+        if (warp == 0) {
+            // ================= TMA producer =========================================================================
+            if (lane == 0 && items > 0) {
+                auto issue_psi = [&](long long g) {
+                    const int s = (int)(g % p.S);
+                    mbar_wait(&tail->empty[s], (uint32_t)(((g / p.S) & 1) ^ 1));
+                    const int it = (int)(g % items), j = it / my_nc, c = it - j * my_nc;
+                    const int tile = cl + j * p.n_clusters;
+                    mbar_arrive_expect_tx(&tail->full[s], (uint32_t)psi_tile_bytes);
+                    tma_load_2d(base + (size_t)s * stage_bytes, &tm_psi, (kc0 + c) * 32, tile * p.AT, &tail->full[s]);
+                };
+                const long long first = (long long)t * items;
+                for (int it = 0; it < items; it++) {
+                    const long long g = first + it;
+                    if (g >= pi) { issue_psi(g); pi = g + 1; }
+                    const int s = (int)(g % p.S);
+                    const int c = it % my_nc;
+                    mbar_arrive_expect_tx(&tail->full[s], (uint32_t)kTcRsTileBytes);
+                    tma_load_2d(base + (size_t)s * stage_bytes + psi_tile_bytes, &tm_rs, (kc0 + c) * 32, 0, &tail->full[s]);
+                    ri = g + 1;
+                }
+                if (t + 1 < p.max_iter) {                                      // the dictionary of the next iteration, ahead of the barriers
+                    const int ahead = items < p.S ? items : p.S;
+                    for (int it = 0; it < ahead; it++) {
+                        const long long g = first + items + it;
+                        if (g >= pi) { issue_psi(g); pi = g + 1; }
+                    }
+                }
+            }
+        } else if (warp == 1) {
+            // ================= MMA issuer ==============================================================================
+            for (int j = 0; j < n_my_tiles; j++) {
+                mbar_wait(&tail->tmem_empty, ((tile_count + j) & 1) ^ 1);      // epilogue of the previous tile has drained TMEM
+                tc_fence_after_sync();
+                for (int c = 0; c < my_nc; c++, g_mma++) {
+                    const int s = (int)(g_mma % p.S), h = (int)(g_mma & 1);
+                    const uint32_t psi_addr = base_u32 + (uint32_t)(s * stage_bytes);
+                    const uint32_t rs_addr = psi_addr + (uint32_t)psi_tile_bytes;
+                    const uint32_t lo_addr = base_u32 + (uint32_t)(p.S * stage_bytes + h * psi_tile_bytes);
+                    mbar_wait(&tail->full[s], (uint32_t)((g_mma / p.S) & 1));
+                    tc_fence_after_sync();
+                    if (lane == 0) {
+#pragma unroll
+                        for (int k = 0; k < 4; k++)
+                            umma_tf32(tmem, umma_smem_desc_sw128(rs_addr + k * 32), umma_smem_desc_sw128(psi_addr + k * 32),
+                                      idesc, (c > 0 || k > 0) ? 1u : 0u);
+                    }
+                    __syncwarp();
+                    mbar_wait(&tail->lo_full[h], (uint32_t)((g_mma >> 1) & 1));
+                    tc_fence_after_sync();
+                    if (lane == 0) {
+#pragma unroll
+                        for (int k = 0; k < 4; k++)
+                            umma_tf32(tmem + 256u, umma_smem_desc_sw128(rs_addr + k * 32), umma_smem_desc_sw128(lo_addr + k * 32),
+                                      idesc, (c > 0 || k > 0) ? 1u : 0u);
+                        umma_commit(&tail->empty[s]);
+                        umma_commit(&tail->lo_empty[h]);
+                        if (c == my_nc - 1) umma_commit(&tail->tmem_full);
+                    }
+                    __syncwarp();
+                }
+            }
+        } else {
+            // ================= workers: dictionary low parts, then the epilogue =========================================
+            const int wtid = tid - 64;
+            const int q4 = warp & 3, half = (warp - 2) >> 2;
+            const int L = q4 * 32 + lane, b_row = L & 63;
+            unsigned long long best = 0ull;
+            for (int j = 0; j < n_my_tiles; j++) {
+                const int tile = cl + j * p.n_clusters;
+                for (int c = 0; c < my_nc; c++, g_wrk++) {
+                    const int s = (int)(g_wrk % p.S), h = (int)(g_wrk & 1);
+                    const float4* raw = reinterpret_cast<const float4*>(base + (size_t)s * stage_bytes);
+                    float4* lo = reinterpret_cast<float4*>(lo_ring + (size_t)h * psi_tile_bytes);
+                    mbar_wait(&tail->full[s], (uint32_t)((g_wrk / p.S) & 1));
+                    mbar_wait(&tail->lo_empty[h], (uint32_t)(((g_wrk >> 1) & 1) ^ 1));
+                    for (int i = wtid; i < p.AT * 8; i += kTcWorkers) {
+                        const float4 v = raw[i];
+                        lo[i] = make_float4(tf32_rn(v.x - tf32_trunc(v.x)), tf32_rn(v.y - tf32_trunc(v.y)),
+                                            tf32_rn(v.z - tf32_trunc(v.z)), tf32_rn(v.w - tf32_trunc(v.w)));
+                    }
+                    fence_proxy_async_smem();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(&tail->lo_full[h]);
+                }
+                // ---- epilogue of this tile: D rows b (hi residual part) + 64+b (lo residual part) -> P[col][b] -----------
+                const unsigned int ph = (tile_count + j) & 1;
+                mbar_wait(&tail->tmem_full, ph);
+                tc_fence_after_sync();
+                const int col0 = half * (p.AT >> 1), col1 = col0 + (p.AT >> 1);
+                const uint32_t trow = tmem + ((uint32_t)(q4 * 32) << 16);
+                if (L >= 64) {
+                    for (int col = col0; col < col1; col += 16) {
+                        float v[16], w[16];
+                        tmem_ld16(trow + (uint32_t)col, v);
+                        tmem_ld16(trow + 256u + (uint32_t)col, w);
+#pragma unroll
+                        for (int i = 0; i < 16; i++) P[(col + i) * 64 + b_row] = v[i] + w[i];
+                    }
+                }
+                named_bar_sync(1, kTcWorkers);
+                if (L < 64) {
+                    for (int col = col0; col < col1; col += 16) {
+                        float v[16], w[16];
+                        tmem_ld16(trow + (uint32_t)col, v);
+                        tmem_ld16(trow + 256u + (uint32_t)col, w);
+#pragma unroll
+                        for (int i = 0; i < 16; i++) P[(col + i) * 64 + b_row] += v[i] + w[i];
+                    }
+                }
+                tc_fence_before_sync();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&tail->tmem_empty);
+                named_bar_sync(1, kTcWorkers);
+                // ---- split-K: exchange the four partial tiles through distributed shared memory ----------------------------
+                if (wtid == 0)
+                    for (uint32_t r = 0; r < kTcCluster; r++) mbar_arrive_cluster(map_to_cta(smem_u32(&tail->cl_ready), r));
+                mbar_wait_cluster(&tail->cl_ready, ph);
+                {
+                    const int b = wtid & 63, g4 = wtid >> 6;
+                    const int per_cta = p.AT >> 2, per_grp = p.AT >> 4;
+                    const int jc0 = (int)q * per_cta + g4 * per_grp;
+                    const uint32_t p_addr = smem_u32(P);
+                    uint32_t pr[kTcCluster];
+#pragma unroll
+                    for (uint32_t r = 0; r < kTcCluster; r++) pr[r] = map_to_cta(p_addr, r);
+                    for (int jc = jc0; jc < jc0 + per_grp; jc++) {
+                        const uint32_t off = (uint32_t)(jc * 64 + b) * 4u;
+                        float v = ld_dsmem_f32(pr[0] + off);
+                        v += ld_dsmem_f32(pr[1] + off);
+                        v += ld_dsmem_f32(pr[2] + off);
+                        v += ld_dsmem_f32(pr[3] + off);
+                        const int atom = tile * p.AT + jc;
+                        if (atom < p.M && b < p.B) {
+                            const unsigned long long k = pack_key(v, atom);
+                            best = k > best ? k : best;
+                            if (p.dbg_C && t == 0) p.dbg_C[(size_t)b * p.M + atom] = v;
+                        }
+                    }
+                }
+                if (n_my_tiles > 1) {                                          // peers must finish reading P before the next tile reuses it
+                    named_bar_sync(1, kTcWorkers);
+                    if (wtid == 0)
+                        for (uint32_t r = 0; r < kTcCluster; r++) mbar_arrive_cluster(map_to_cta(smem_u32(&tail->cl_done), r));
+                    mbar_wait_cluster(&tail->cl_done, ph);
+                }
+            }
+            // ---- per-signal argmax of this CTA -> grid-wide key slot of iteration t --------------------------------------------
+            tail->skeys[wtid] = best;
+            named_bar_sync(1, kTcWorkers);
+            if (wtid < 64 && wtid < p.B && n_my_tiles > 0) {
+                unsigned long long k = tail->skeys[wtid];
+#pragma unroll
+                for (int g4 = 1; g4 < 4; g4++) { const unsigned long long o = tail->skeys[g4 * 64 + wtid]; k = o > k ? o : k; }
+                if (k) red_max_u64(p.keys + (t % 3) * 64 + wtid, k);
+            }
+        }
+        tile_count += (unsigned int)n_my_tiles;
+        tc_grid_barrier(p.ctrl, ++episode * (unsigned long long)G);
+
+        // ================= owners: Eq. 10, Eq. 11, Eq. 18, per-signal stop test ==================================================
+        for (int b = blockIdx.x; b < p.B; b += G) {
+            if (!p.state[b].active) continue;
+            const unsigned long long key = ld_relaxed_u64(p.keys + (t % 3) * 64 + b);
+            const int i = key_index(key);
+            const float c = key_value(key);
+            const double cd = (double)c;
+            const float* psi_i = p.psi_t + (int64_t)i * p.ld;
+            double s2 = 0.0;
+            for (int n = tid; n < p.N; n += kTcThreads) {
+                const double v = p.r64[(size_t)b * p.Nr + n] - cd * (double)__ldg(psi_i + n);
+                tc_publish(p, b, n, v);
+                s2 += v * v;
+            }
+            const double rr = tc_block_sum(s2, tail->red);
+            const bool done = !(sqrt(rr) > p.state[b].thresh) || (t + 1 >= p.max_iter);
+            if (done)
+                for (int n = tid; n < p.N; n += kTcThreads) p.R[(size_t)b * p.N + n] = (float)p.r64[(size_t)b * p.Nr + n];
+            __syncthreads();                                                    // every thread has read state[b] before it changes
+            if (tid == 0) {
+                p.x64[(size_t)b * p.M + i] += cd;
+                if (p.idx_trace) p.idx_trace[(size_t)b * p.ldt + t] = i;
+                if (p.c_trace) p.c_trace[(size_t)b * p.ldt + t] = c;
+                st_relaxed_u64(p.keys + ((t + 2) % 3) * 64 + b, 0ull);          // slot of iteration t-1, reused at t+2
+                if (done) {
+                    p.n_iter[b] = t + 1;
+                    p.state[b].active = 0;
+                    atomicAdd(p.ctrl + 5, ~0ull);                               // one signal fewer
+                }
+            }
+        }
+        tc_grid_barrier(p.ctrl, ++episode * (unsigned long long)G);
+        if (tid == 0) tail->n_active = (int)ld_acquire_u64(p.ctrl + 5);
+        __syncthreads();
+        n_active = tail->n_active;
+        t += 1;
+    }
+
+    // ---- dictionary tiles prefetched for an iteration that never ran: let them land --------------------------------------------
+    if (warp == 0 && lane == 0) {
+        for (long long g = ri; g < pi; g++) {
+            const int s = (int)(g % p.S);
+            mbar_arrive(&tail->full[s]);
+            mbar_wait(&tail->full[s], (uint32_t)((g / p.S) & 1));
+        }
+    }
+    // ---- P:86 return x~ ------------------------------------------------------------------------------------------------------------
+    for (size_t idx = (size_t)blockIdx.x * kTcThreads + tid; idx < (size_t)p.B * p.M; idx += (size_t)G * kTcThreads)
+        p.X[idx] = (float)__ldcg(p.x64 + idx);
+
+    tc_fence_before_sync();
+    __syncthreads();
+    cluster_sync_all();                                                          // nobody still reads this CTA's shared memory
+    if (warp == 1) tmem_dealloc(tmem, kTcTmemCols);
+}
+
+// ------------------------------------------------------------------------------------------------------------------------------------
+// host side
+// ------------------------------------------------------------------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static mp_status encode_fn(EncodeTiledFn* out)
+{
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void* sym = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        MP_CUDA(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &sym, cudaEnableDefault, &qres));
+        if (qres != cudaDriverEntryPointSuccess || !sym) return fail(MP_ERR_UNSUPPORTED, "cuTensorMapEncodeTiled is not available");
+        fn = reinterpret_cast<EncodeTiledFn>(sym);
+    }
+    *out = fn;
+    return MP_OK;
+}
+
+// fp32 matrix, rows x cols, row pitch ld floats; box = box_rows x 32 floats, 128-byte swizzle, out-of-bounds reads give 0
+static mp_status make_map(CUtensorMap* map, const float* ptr, uint64_t rows, uint64_t cols, uint64_t ld, uint32_t box_rows)
+{
+    EncodeTiledFn fn;
+    mp_status st = encode_fn(&fn);
+    if (st != MP_OK) return st;
+    const cuuint64_t gdim[2] = {cols, rows};
+    const cuuint64_t gstride[1] = {ld * sizeof(float)};
+    const cuuint32_t box[2] = {32, box_rows};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float*>(ptr), gdim, gstride, box, estr,
+                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(MP_ERR_CUDA, "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
+    return MP_OK;
+}
+
+struct TcPlan {
+    int AT, n_tiles, n_clusters, tiles_per_cluster, nchunks, S;
+    size_t smem;
+};
+
+static mp_status tc_max_clusters(size_t smem, int* out)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(kTcCluster * 64);
+    cfg.blockDim = dim3(kTcThreads);
+    cfg.dynamicSmemBytes = smem;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = kTcCluster; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    int n = 0;
+    MP_CUDA(cudaOccupancyMaxActiveClusters(&n, mp_batched_tc_kernel, &cfg));
+    *out = n;
+    return MP_OK;
+}
+
+static mp_status tc_plan(int N, int M, int B, const DeviceInfo& di, TcPlan* plan)
+{
+    if (B > 64) return fail(MP_ERR_UNSUPPORTED, "tensor-core batched path takes at most 64 signals per launch");
+    const int nchunks = (N + 31) / 32;
+    if (nchunks < kTcCluster) return fail(MP_ERR_UNSUPPORTED, "N=%d is too short for the split-K tensor-core path", N);
+    static thread_local int attr_dev = -1;
+    if (attr_dev != di.device) {
+        MP_CUDA(cudaFuncSetAttribute(mp_batched_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, di.smem_optin));
+        attr_dev = di.device;
+    }
+    static thread_local int cached_dev = -1, cached_clusters = 0;
+    if (cached_dev != di.device) {
+        int n = 0;
+        mp_status st = tc_max_clusters((size_t)di.smem_optin, &n);
+        if (st != MP_OK) return st;
+        cached_clusters = n; cached_dev = di.device;
+    }
+    int C = cached_clusters;
+    if (options().grid > 0 && options().grid / kTcCluster < C) C = (int)options().grid / kTcCluster;
+    if (C < 1) return fail(MP_ERR_UNSUPPORTED, "no cluster of %d CTAs fits on this device", kTcCluster);
+    if ((int64_t)C * kTcCluster < B) return fail(MP_ERR_UNSUPPORTED, "fewer co-resident CTAs than signals");
+    int AT = round_up((M + C - 1) / C, 32);
+    if (AT > 256) AT = 256;
+    if (AT < 32) AT = 32;
+    plan->AT = AT;
+    plan->n_tiles = (M + AT - 1) / AT;
+    plan->n_clusters = C;
+    plan->tiles_per_cluster = (plan->n_tiles + C - 1) / C;
+    plan->nchunks = nchunks;
+    const size_t stage = (size_t)AT * 128 + kTcRsTileBytes;
+    const size_t fixed = 1024 + 2 * (size_t)AT * 128 + sizeof(TcTail) + 64;
+    if (fixed + 2 * stage > (size_t)di.smem_optin) return fail(MP_ERR_UNSUPPORTED, "shared memory too small for the tensor-core path");
+    int S = (int)(((size_t)di.smem_optin - fixed) / stage);
+    if (S > kTcMaxStages) S = kTcMaxStages;
+    if (options().depth > 0 && options().depth < S && options().depth >= 2) S = (int)options().depth;
+    plan->S = S;
+    plan->smem = fixed + (size_t)S * stage;
+    return MP_OK;
+}
+
+bool batched_tc_supported(int N, int M, int B)
+{
+    DeviceInfo di;
+    if (device_info(&di) != MP_OK) return false;
+    TcPlan plan;
+    return tc_plan(N, M, B, di, &plan) == MP_OK;
+}
+
+mp_status launch_recover_batched_tc(const BatchedArgs& a, const Workspace& ws, float* dbg_C, cudaStream_t stream)
+{
+    DeviceInfo di;
+    mp_status st = device_info(&di);
+    if (st != MP_OK) return st;
+    TcPlan plan;
+    st = tc_plan(a.N, a.M, a.B, di, &plan);
+    if (st != MP_OK) return st;
+    const int Nr = round_up(a.N, 128);
+
+    CUtensorMap tm_psi, tm_rs;
+    st = make_map(&tm_psi, a.psi_t, (uint64_t)a.M, (uint64_t)a.N, (uint64_t)a.ld, (uint32_t)plan.AT);
+    if (st != MP_OK) return st;
+    st = make_map(&tm_rs, ws.rs, 128, (uint64_t)a.N, (uint64_t)Nr, 128);
+    if (st != MP_OK) return st;
+
+    // control block + float64 coefficient accumulators (Eq. 8), argmax key slots, hi/lo residual rows (rows >= B stay 0)
+    MP_CUDA(cudaMemsetAsync(ws.ctrl, 0, 256 + sizeof(double) * (size_t)a.B * a.M, stream));
+    MP_CUDA(cudaMemsetAsync(ws.keys, 0, sizeof(unsigned long long) * 3 * 64, stream));
+    MP_CUDA(cudaMemsetAsync(ws.rs, 0, sizeof(float) * 128 * (size_t)Nr, stream));
+
+    BatchedTcParams p;
+    p.psi_t = a.psi_t; p.ld = a.ld; p.Y = a.Y; p.ldy = a.ldy;
+    p.X = a.X; p.R = a.R; p.n_iter = a.n_iter; p.idx_trace = a.idx_trace; p.c_trace = a.c_trace; p.ldt = a.ldt;
+    p.x64 = ws.x64; p.r64 = ws.r64; p.rs = ws.rs; p.ctrl = ws.ctrl; p.keys = ws.keys;
+    p.state = reinterpret_cast<SigState*>(ws.state);
+    p.dbg_C = dbg_C;
+    p.N = a.N; p.M = a.M; p.B = a.B; p.Nr = Nr; p.Npad = round_up(a.N, 4);
+    p.AT = plan.AT; p.n_tiles = plan.n_tiles; p.n_clusters = plan.n_clusters; p.tiles_per_cluster = plan.tiles_per_cluster;
+    p.nchunks = plan.nchunks; p.S = plan.S;
+    p.eps = a.eps; p.max_iter = a.max_iter;
+
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(plan.n_clusters * kTcCluster);
+    cfg.blockDim = dim3(kTcThreads);
+    cfg.dynamicSmemBytes = plan.smem;
+    cfg.stream = stream;
+    cudaLaunchAttribute at[2];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = kTcCluster; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    at[1].id = cudaLaunchAttributeCooperative;
+    at[1].val.cooperative = 1;
+    cfg.attrs = at; cfg.numAttrs = 2;
+    cudaError_t e = cudaLaunchKernelEx(&cfg, mp_batched_tc_kernel, tm_psi, tm_rs, p);
+    if (e == cudaErrorNotSupported || e == cudaErrorInvalidValue || e == cudaErrorCooperativeLaunchTooLarge) {
+        // cluster + cooperative attribute refused: the grid is sized from cudaOccupancyMaxActiveClusters, so all
+        // clusters are co-resident on an otherwise idle device without the attribute as well
+        (void)cudaGetLastError();
+        cfg.numAttrs = 1;
+        e = cudaLaunchKernelEx(&cfg, mp_batched_tc_kernel, tm_psi, tm_rs, p);
+    }
+    if (e != cudaSuccess) return cuda_fail(e, "cudaLaunchKernelEx(mp_batched_tc_kernel)");
+    count_launch();
+    return MP_OK;
+}
+
+}  // namespace mp

@@ -39,7 +39,8 @@ struct Workspace {
     double* r64;                // B*Nr   (Nr = N rounded up to 128)
     float* r32;                 // B*Nr
     unsigned long long* keys;   // 3*B  rotating per-signal key slots (batched)
-    int* state;                 // B    per-signal: 1 = active
+    int* state;                 // 4*B ints: per-signal stop state of the batched kernel
+    float* rs;                  // 128*Nr  (B > 1 only) hi / lo split of the fp32 residuals, the tensor-core A operand
     size_t bytes;
 };
 size_t workspace_layout(int N, int M, int B, void* base, Workspace* ws);
@@ -64,5 +65,8 @@ struct BatchedArgs {
     int* idx_trace; float* c_trace; int64_t ldt;
 };
 mp_status launch_recover_batched(const BatchedArgs& a, const Workspace& ws, cudaStream_t stream);
+// tensor-core lock-step kernel (B <= 64 per launch); dbg_C (nullable, B x M) receives the correlations of iteration 0
+mp_status launch_recover_batched_tc(const BatchedArgs& a, const Workspace& ws, float* dbg_C, cudaStream_t stream);
+bool batched_tc_supported(int N, int M, int B);
 
 }  // namespace mp

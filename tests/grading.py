@@ -3,8 +3,9 @@
 Implements the parity contract of BASELINE.json's north_star under the readings listed in DESIGN.md:
 
   G1 free-running: the GPU index sequence equals the oracle's up to the first iteration whose top-two
-     relative gap of |c| (on the oracle's own state) is <= 1e-4 -- after a legal near-tie flip the two
-     runs are different trajectories and cannot be compared step by step.
+     relative gap of |c| (on the oracle's own state) is <= 1e-4 plus the drift allowance 2 ||d|| / max|c|,
+     d = the difference of the two residuals accumulated from the step-value errors so far (each bounded by G3)
+     -- after a legal near-tie flip the two runs are different trajectories and cannot be compared step by step.
   G2 teacher-forced replay over the WHOLE GPU trace: the oracle is advanced with the GPU's own (index,
      step) pairs, so its state is the exact-arithmetic image of the GPU state; at every iteration the
      GPU's pick must be the oracle's argmax, or a near-tie (gap <= 1e-4 and |c_ref[pick]| >= (1-1e-4) max).
@@ -67,8 +68,20 @@ def grade_single(psi32: np.ndarray, y32: np.ndarray, eps: float, max_iter: int,
     diff = np.nonzero(idx_gpu[:L] != ref.idx[:L])[0]
     first_div = int(diff[0]) if diff.size else -1
     if first_div >= 0:
-        assert ref.gap[first_div] <= GAP_TOL, (
-            f"free-running sequences diverge at t={first_div} where the oracle's top-two gap is {ref.gap[first_div]:.3e} > {GAP_TOL}")
+        # The oracle's gap is measured on the ORACLE's state; the GPU decided on ITS state.  Up to first_div both
+        # took the same atoms, so the two residuals differ only by the accumulated step-value errors (each within
+        # C_TOL ||r_s||, G3): d = sum_s (c_gpu,s - c_ref,s) psi_idx_s.  Every correlation then differs by at most
+        # ||d|| (unit atoms), which moves the top-two comparison by at most 2 ||d|| / max|c|.  A divergence is legal
+        # if the oracle's gap is within GAP_TOL plus that drift allowance; G2 below still requires the GPU's pick
+        # to be the argmax (or a <= 1e-4 near-tie) of the exact-arithmetic image of its own state at EVERY step.
+        d = np.zeros(N)
+        for s_ in range(first_div):
+            d += (c_gpu[s_] - ref.c[s_]) * psi32[idx_gpu[s_]].astype(np.float64)
+        cmax = abs(ref.c[first_div])
+        allowance = GAP_TOL + 2.0 * float(np.linalg.norm(d)) / max(cmax, np.finfo(np.float64).tiny)
+        assert ref.gap[first_div] <= allowance, (
+            f"free-running sequences diverge at t={first_div} where the oracle's top-two gap is {ref.gap[first_div]:.3e} "
+            f"> {GAP_TOL} + state-drift allowance {allowance - GAP_TOL:.3e}")
 
     # ---- G2/G3 teacher-forced replay ------------------------------------------------------------------------
     rp = oracle.mp_replay(psi32, y, idx_gpu, c_gpu, nthreads)

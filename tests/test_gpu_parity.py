@@ -236,13 +236,41 @@ def test_cfg3_full_size_sampled_grading(mp):
 
 
 # ------------------------------------------------------------------------------------------ batched (a9)
-@pytest.mark.parametrize("B,N,M,K", [(3, 256, 1024, 16), (5, 250, 333, 8), (64, 128, 512, 6)])
-def test_batched_every_signal_graded_like_a_single_run(mp, B, N, M, K):
+BATCHED_ALGOS = [1, 2]        # 1 = lock-step tensor-core kernel (split-TF32 tcgen05), 2 = sequential single-signal solves
+
+
+@pytest.mark.parametrize("B,N,M", [(64, 2048, 8192), (7, 250, 333), (64, 128, 512), (1, 4096, 2048), (33, 1000, 9000)])
+def test_batched_correlation_matches_float64_oracle(mp, B, N, M):
+    """The contraction of the batched path alone: C = Psi^T Y on the tensor cores against the oracle's float64
+    ascending-n dot products (Eq. 9), every element, tolerance C_TOL * ||y_b||."""
+    cfg = problems.custom_config(N, M, max(1, N // 16), B=B)
+    psi32 = problems.normalise_on_host(synth.make_dictionary(cfg, seed=11))
+    rng = np.random.default_rng(5)
+    Y = rng.standard_normal((B, N)).astype(np.float32)
+    Y[:, ::7] *= 1e-3                                                        # mixed magnitudes inside one residual
+    ld = (N + 3) // 4 * 4
+    buf = torch.full((M, ld), 3.0, dtype=torch.float32, device="cuda"); buf[:, :N] = dev(psi32)
+    Yb = torch.full((B, ld), -2.0, dtype=torch.float32, device="cuda"); Yb[:, :N] = dev(Y)
+    Cg = mp.mp_correlate_batched(buf[:, :N], Yb[:, :N])
+    torch.cuda.synchronize()
+    Cg = Cg.cpu().numpy().astype(np.float64)
+    worst = 0.0
+    for b in range(B):
+        ref = oracle.correlate(psi32, Y[b].astype(np.float64), nthreads=oracle.default_threads())
+        err = np.abs(Cg[b] - ref).max() / np.linalg.norm(Y[b].astype(np.float64))
+        worst = max(worst, err)
+    assert worst <= grading.C_TOL, worst
+
+
+@pytest.mark.parametrize("algo", BATCHED_ALGOS)
+@pytest.mark.parametrize("B,N,M,K", [(3, 256, 1024, 16), (5, 250, 333, 8), (64, 128, 512, 6), (9, 512, 9000, 24)])
+def test_batched_every_signal_graded_like_a_single_run(mp, B, N, M, K, algo):
     """P:165 / reading R17: signal b's result is MP on (Psi, y_b) under the same rules as the single-signal path
     (full teacher-forced grading per signal through the traced entry point); finished signals are frozen."""
     cfg = problems.custom_config(N, M, K, eps=1e-5, max_iter=10 * K, B=B)
     pb = problems.make_problem(cfg, seed=6)
     pb.Y[B // 2] = 0.0                                                       # one signal that stops at once
+    mp.mp_set_int("batched_algo", algo)
     ld = (N + 3) // 4 * 4
     buf = torch.full((M, ld), 5.0, dtype=torch.float32, device="cuda"); buf[:, :N] = dev(pb.psi32)
     Yb = torch.full((B, ld), 9.0, dtype=torch.float32, device="cuda"); Yb[:, :N] = dev(pb.Y)
