@@ -179,6 +179,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--max-iter", type=int, default=None, help="override the config's iteration cap (profiling runs)")
+    ap.add_argument("--knob", action="append", default=[], metavar="NAME=VALUE", help="mp_set_int knob (profiling runs)")
     args = ap.parse_args()
     cfg = synth.config(args.config)
     if args.max_iter is not None:
@@ -191,6 +192,9 @@ def main():
     import torch
     import paper_0809_1833_b200 as mp   # raises if the CUDA library is missing: there is no fallback
 
+    for kv in args.knob:
+        name, _, val = kv.partition("=")
+        mp.mp_set_int(name, int(val))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
@@ -308,6 +312,9 @@ def main():
 
 def mp_kernel_name(mp):
     try:
+        if mp.mp_get_int("info_tc_clusters"):
+            return ("mp_batched_tc_kernel (%d clusters x 4 CTAs, %d atoms/tile, %d stages)"
+                    % (mp.mp_get_int("info_tc_clusters"), mp.mp_get_int("info_tc_at"), mp.mp_get_int("info_tc_stages")))
         return {0: "auto", 1: "mp_persistent_kernel", 2: "stream loop"}[mp.mp_get_int("algo")]
     except Exception:
         return "?"

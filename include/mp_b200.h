@@ -130,7 +130,9 @@ MP_API const char* mp_last_error(void);
  *   "grid"          CTAs of the persistent kernel (0 = auto = one per SM)
  *   "chunk"         iterations enqueued between stop-flag polls of algo 2 (default 64)
  *   "batched_algo"  0 = auto (default): lock-step tensor-core kernel in groups of <= 64 signals when the shape fits,
- *                   1 = tensor-core kernel or MP_ERR_UNSUPPORTED, 2 = one single-signal solve after another */
+ *                   1 = tensor-core kernel or MP_ERR_UNSUPPORTED, 2 = one single-signal solve after another
+ *   "batched_coop"  1 (default) = launch the batched kernel with the cooperative attribute (co-residency checked by
+ *                   the driver), 0 = plain cluster launch of a grid sized from cudaOccupancyMaxActiveClusters */
 MP_API mp_status mp_set_int(const char* name, int64_t value);
 MP_API mp_status mp_get_int(const char* name, int64_t* value);
 

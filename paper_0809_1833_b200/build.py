@@ -30,7 +30,7 @@ def deps():
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in deps()):
         return LIB
-    flags = [f for f in FLAGS if not f.startswith("--use_fast_math")]
+    flags = [f for f in FLAGS if not f.startswith("--use_fast_math")] + os.environ.get("MP_B200_EXTRA_NVCC_FLAGS", "").split()
     if verbose:
         flags += ["-Xptxas", "-v"]
     objs = []

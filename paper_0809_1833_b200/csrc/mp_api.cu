@@ -131,6 +131,10 @@ static int64_t* option_slot(const char* name)
     if (!strcmp(name, "grid")) return &o.grid;
     if (!strcmp(name, "chunk")) return &o.chunk;
     if (!strcmp(name, "batched_algo")) return &o.batched_algo;
+    if (!strcmp(name, "batched_coop")) return &o.batched_coop;
+    if (!strcmp(name, "info_tc_clusters")) return &o.info_tc_clusters;
+    if (!strcmp(name, "info_tc_at")) return &o.info_tc_at;
+    if (!strcmp(name, "info_tc_stages")) return &o.info_tc_stages;
     return nullptr;
 }
 

@@ -35,21 +35,35 @@ constexpr int kTcWorkers = 256;
 constexpr int kTcCluster = 4;            // split-K ways
 constexpr int kTcMaxStages = 8;
 constexpr int kTcRsTileBytes = 128 * 128;
+constexpr int kTcRegElems = 8;           // float64 residual elements an owner thread keeps in registers (N <= 2560), else global
 constexpr uint32_t kTcTmemCols = 512;    // two accumulators: columns [0, AT) dictionary-hi products, [256, 256 + AT) dictionary-lo products
 
-struct SigState {
-    double thresh;                       // eps * ||y_b||
-    int active, pad;
-};
+// Optional phase timeline (profiling builds only, -DMP_TC_TIMING): globaltimer stamps of a few CTAs per iteration.
+#ifdef MP_TC_TIMING
+constexpr int kTcStampIters = 64, kTcStampCtas = 4, kTcStampSlots = 9;
+__device__ unsigned long long g_tc_stamps[kTcStampCtas][kTcStampIters][kTcStampSlots];
+__device__ __forceinline__ unsigned long long tc_now()
+{
+    unsigned long long v;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(v));
+    return v;
+}
+#define TC_STAMP(cond, slot)                                                                                   \
+    do {                                                                                                       \
+        if ((cond) && t < kTcStampIters && (blockIdx.x % 37) == 0 && blockIdx.x / 37 < kTcStampCtas)           \
+            g_tc_stamps[blockIdx.x / 37][t][slot] = tc_now();                                                  \
+    } while (0)
+#else
+#define TC_STAMP(cond, slot) do {} while (0)
+#endif
 
 struct BatchedTcParams {
     const float* psi_t; int64_t ld;
     const float* Y; int64_t ldy;
     float* X; float* R; int* n_iter; int* idx_trace; float* c_trace; int64_t ldt;
     double* x64; double* r64; float* rs;            // rs: [128][Nr]  rows 0-63 hi parts, rows 64-127 lo parts
-    unsigned long long* ctrl;                       // [0] grid-barrier counter, [5] number of active signals
+    unsigned long long* ctrl;                       // [0] grid-barrier counter, [5] number of active signals, [16] CTAs whose keys are out
     unsigned long long* keys;                       // [3][64] rotating per-signal argmax keys
-    SigState* state;
     float* dbg_C;                                   // nullable: B x M correlations of iteration 0 (mp_correlate_batched)
     int N, M, B, Nr, Npad;
     int AT, n_tiles, n_clusters, tiles_per_cluster, nchunks, S;
@@ -66,16 +80,12 @@ struct TcTail {
 
 __device__ __forceinline__ void tc_grid_barrier(unsigned long long* counter, unsigned long long target)
 {
-    fence_proxy_async_all();            // this thread's global writes (residual rows) are later read by TMA in other CTAs
     __syncthreads();
     if (threadIdx.x == 0) {
-        __threadfence();
-        red_add_release_u64(counter, 1ull);
+        red_add_release_u64(counter, 1ull);             // cumulative: covers the CTA's writes ordered by the bar.sync above
         while (ld_acquire_u64(counter) < target) {}
-        __threadfence();
     }
     __syncthreads();
-    fence_proxy_async_all();            // residual rows written by other CTAs are read by TMA (async proxy) next
 }
 
 // Split-TF32 operands.  kind::tf32 reads fp32 words and uses their top 19 bits (sign, exponent, 10 mantissa bits).
@@ -106,12 +116,11 @@ __device__ __forceinline__ double tc_block_sum(double v, double* red)
     return s;
 }
 
-// writes r (float64) and the hi / lo split of its fp32 rounding
+// publishes the hi / lo split of the fp32 rounding of one residual element (the tensor-core A operand rows b, 64+b)
 __device__ __forceinline__ void tc_publish(const BatchedTcParams& p, int b, int n, double v)
 {
     const float f = (float)v;
     const float hi = tf32_rn(f);
-    p.r64[(size_t)b * p.Nr + n] = v;
     p.rs[(size_t)b * p.Nr + n] = hi;
     p.rs[(size_t)(64 + b) * p.Nr + n] = tf32_rn(f - hi);
 }
@@ -162,24 +171,45 @@ mp_batched_tc_kernel(const __grid_constant__ CUtensorMap tm_psi, const __grid_co
     const int items = n_my_tiles * my_nc;                                      // pipeline items per MP iteration
     const uint32_t idesc = umma_idesc_tf32(128, p.AT);
 
-    // ---- Eq. 8 for every signal: r_b <- y_b, ||y_b||, per-signal stop state ------------------------------------------
-    for (int b = blockIdx.x; b < p.B; b += G) {
+    // ---- Eq. 8: CTA b owns signal b (B <= 64 <= gridDim).  r_b <- y_b in float64 (registers of the owner's threads when
+    //      N <= 2560, else the workspace), ||y_b||, the stop threshold; hi / lo rows of the residual operand ------------
+    const int b_own = blockIdx.x;
+    const bool owner = b_own < p.B;
+    const bool reg_r = p.Nr <= kTcRegElems * kTcThreads;
+    double rreg[kTcRegElems];
+    double thresh = 0.0;
+    bool my_active = false;
+#pragma unroll
+    for (int k = 0; k < kTcRegElems; k++) rreg[k] = 0.0;
+    if (owner) {
         double ss = 0.0;
-        for (int n = tid; n < p.Nr; n += kTcThreads) {
-            const double v = n < p.N ? (double)p.Y[(size_t)b * p.ldy + n] : 0.0;
-            tc_publish(p, b, n, v);
-            ss += v * v;
+        if (reg_r) {
+#pragma unroll
+            for (int k = 0; k < kTcRegElems; k++) {
+                const int n = tid + k * kTcThreads;
+                if (n < p.N) {
+                    const double v = (double)p.Y[(size_t)b_own * p.ldy + n];
+                    rreg[k] = v;
+                    tc_publish(p, b_own, n, v);
+                    ss += v * v;
+                }
+            }
+        } else {
+            for (int n = tid; n < p.N; n += kTcThreads) {
+                const double v = (double)p.Y[(size_t)b_own * p.ldy + n];
+                p.r64[(size_t)b_own * p.Nr + n] = v;
+                tc_publish(p, b_own, n, v);
+                ss += v * v;
+            }
         }
+        fence_proxy_async_all();                        // the rows are read by TMA (async proxy) in every CTA
         const double yy = tc_block_sum(ss, tail->red);
-        const double thresh = (double)p.eps * sqrt(yy);
-        const bool active = (sqrt(yy) > thresh) && p.max_iter > 0;
-        if (!active) {
-            for (int n = tid; n < p.N; n += kTcThreads) p.R[(size_t)b * p.N + n] = p.Y[(size_t)b * p.ldy + n];
-        }
+        thresh = (double)p.eps * sqrt(yy);
+        my_active = (sqrt(yy) > thresh) && p.max_iter > 0;
+        if (!my_active)
+            for (int n = tid; n < p.N; n += kTcThreads) p.R[(size_t)b_own * p.N + n] = p.Y[(size_t)b_own * p.ldy + n];
         if (tid == 0) {
-            p.state[b].thresh = thresh;
-            p.state[b].active = active ? 1 : 0;
-            if (active) atomicAdd(p.ctrl + 5, 1ull); else p.n_iter[b] = 0;
+            if (my_active) atomicAdd(p.ctrl + 5, 1ull); else p.n_iter[b_own] = 0;
         }
     }
     unsigned long long episode = 0;
@@ -194,6 +224,7 @@ mp_batched_tc_kernel(const __grid_constant__ CUtensorMap tm_psi, const __grid_co
     int t = 0;
 
     while (n_active > 0 && t < p.max_iter) {
+        TC_STAMP(tid == 0, 0);
         if (warp == 0) {
             // ================= TMA producer =========================================================================
             if (lane == 0 && items > 0) {
@@ -206,6 +237,7 @@ mp_batched_tc_kernel(const __grid_constant__ CUtensorMap tm_psi, const __grid_co
                     tma_load_2d(base + (size_t)s * stage_bytes, &tm_psi, (kc0 + c) * 32, tile * p.AT, &tail->full[s]);
                 };
                 const long long first = (long long)t * items;
+                fence_proxy_async_all();                                       // residual rows written by the owners (generic proxy)
                 for (int it = 0; it < items; it++) {
                     const long long g = first + it;
                     if (g >= pi) { issue_psi(g); pi = g + 1; }
@@ -279,39 +311,44 @@ mp_batched_tc_kernel(const __grid_constant__ CUtensorMap tm_psi, const __grid_co
                     __syncwarp();
                     if (lane == 0) mbar_arrive(&tail->lo_full[h]);
                 }
+                TC_STAMP(wtid == 0, 1);
                 // ---- epilogue of this tile: D rows b (hi residual part) + 64+b (lo residual part) -> P[col][b] -----------
                 const unsigned int ph = (tile_count + j) & 1;
                 mbar_wait(&tail->tmem_full, ph);
+                TC_STAMP(wtid == 0, 2);
                 tc_fence_after_sync();
                 const int col0 = half * (p.AT >> 1), col1 = col0 + (p.AT >> 1);
                 const uint32_t trow = tmem + ((uint32_t)(q4 * 32) << 16);
                 if (L >= 64) {
                     for (int col = col0; col < col1; col += 16) {
-                        float v[16], w[16];
-                        tmem_ld16(trow + (uint32_t)col, v);
-                        tmem_ld16(trow + 256u + (uint32_t)col, w);
+                        uint32_t v[16], w[16];
+                        tmem_ld16_issue(trow + (uint32_t)col, v);
+                        tmem_ld16_issue(trow + 256u + (uint32_t)col, w);
+                        tmem_ld_wait(); tmem_ld_pin(v); tmem_ld_pin(w);
 #pragma unroll
-                        for (int i = 0; i < 16; i++) P[(col + i) * 64 + b_row] = v[i] + w[i];
+                        for (int i = 0; i < 16; i++) P[(col + i) * 64 + b_row] = __uint_as_float(v[i]) + __uint_as_float(w[i]);
                     }
                 }
                 named_bar_sync(1, kTcWorkers);
                 if (L < 64) {
                     for (int col = col0; col < col1; col += 16) {
-                        float v[16], w[16];
-                        tmem_ld16(trow + (uint32_t)col, v);
-                        tmem_ld16(trow + 256u + (uint32_t)col, w);
+                        uint32_t v[16], w[16];
+                        tmem_ld16_issue(trow + (uint32_t)col, v);
+                        tmem_ld16_issue(trow + 256u + (uint32_t)col, w);
+                        tmem_ld_wait(); tmem_ld_pin(v); tmem_ld_pin(w);
 #pragma unroll
-                        for (int i = 0; i < 16; i++) P[(col + i) * 64 + b_row] += v[i] + w[i];
+                        for (int i = 0; i < 16; i++) P[(col + i) * 64 + b_row] += __uint_as_float(v[i]) + __uint_as_float(w[i]);
                     }
                 }
                 tc_fence_before_sync();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&tail->tmem_empty);
                 named_bar_sync(1, kTcWorkers);
+                TC_STAMP(wtid == 0, 3);
                 // ---- split-K: exchange the four partial tiles through distributed shared memory ----------------------------
-                if (wtid == 0)
-                    for (uint32_t r = 0; r < kTcCluster; r++) mbar_arrive_cluster(map_to_cta(smem_u32(&tail->cl_ready), r));
+                if (wtid < kTcCluster) mbar_arrive_cluster(map_to_cta(smem_u32(&tail->cl_ready), (uint32_t)wtid));
                 mbar_wait_cluster(&tail->cl_ready, ph);
+                TC_STAMP(wtid == 0, 4);
                 {
                     const int b = wtid & 63, g4 = wtid >> 6;
                     const int per_cta = p.AT >> 2, per_grp = p.AT >> 4;
@@ -320,30 +357,41 @@ mp_batched_tc_kernel(const __grid_constant__ CUtensorMap tm_psi, const __grid_co
                     uint32_t pr[kTcCluster];
 #pragma unroll
                     for (uint32_t r = 0; r < kTcCluster; r++) pr[r] = map_to_cta(p_addr, r);
-                    for (int jc = jc0; jc < jc0 + per_grp; jc++) {
-                        const uint32_t off = (uint32_t)(jc * 64 + b) * 4u;
-                        float v = ld_dsmem_f32(pr[0] + off);
-                        v += ld_dsmem_f32(pr[1] + off);
-                        v += ld_dsmem_f32(pr[2] + off);
-                        v += ld_dsmem_f32(pr[3] + off);
-                        const int atom = tile * p.AT + jc;
-                        if (atom < p.M && b < p.B) {
-                            const unsigned long long k = pack_key(v, atom);
-                            best = k > best ? k : best;
-                            if (p.dbg_C && t == 0) p.dbg_C[(size_t)b * p.M + atom] = v;
+                    for (int jb = jc0; jb < jc0 + per_grp; jb += 8) {          // per_grp = AT/16 is 2, 4, 6, ... : batches of <= 8
+                        const int nb = min(8, jc0 + per_grp - jb);
+                        float part[kTcCluster][8];
+#pragma unroll
+                        for (int u = 0; u < 8; u++) {
+                            if (u < nb) {
+                                const uint32_t off = (uint32_t)((jb + u) * 64 + b) * 4u;
+#pragma unroll
+                                for (int r = 0; r < kTcCluster; r++) part[r][u] = ld_dsmem_f32_nv(pr[r] + off);
+                            }
+                        }
+#pragma unroll
+                        for (int u = 0; u < 8; u++) {
+                            if (u < nb) {
+                                const float v = ((part[0][u] + part[1][u]) + part[2][u]) + part[3][u];   // rank order: deterministic
+                                const int atom = tile * p.AT + jb + u;
+                                if (atom < p.M && b < p.B) {
+                                    const unsigned long long k = pack_key(v, atom);
+                                    best = k > best ? k : best;
+                                    if (p.dbg_C && t == 0) p.dbg_C[(size_t)b * p.M + atom] = v;
+                                }
+                            }
                         }
                     }
                 }
                 if (n_my_tiles > 1) {                                          // peers must finish reading P before the next tile reuses it
                     named_bar_sync(1, kTcWorkers);
-                    if (wtid == 0)
-                        for (uint32_t r = 0; r < kTcCluster; r++) mbar_arrive_cluster(map_to_cta(smem_u32(&tail->cl_done), r));
+                    if (wtid < kTcCluster) mbar_arrive_cluster(map_to_cta(smem_u32(&tail->cl_done), (uint32_t)wtid));
                     mbar_wait_cluster(&tail->cl_done, ph);
                 }
             }
             // ---- per-signal argmax of this CTA -> grid-wide key slot of iteration t --------------------------------------------
             tail->skeys[wtid] = best;
             named_bar_sync(1, kTcWorkers);
+            TC_STAMP(wtid == 0, 5);
             if (wtid < 64 && wtid < p.B && n_my_tiles > 0) {
                 unsigned long long k = tail->skeys[wtid];
 #pragma unroll
@@ -352,40 +400,75 @@ mp_batched_tc_kernel(const __grid_constant__ CUtensorMap tm_psi, const __grid_co
             }
         }
         tile_count += (unsigned int)n_my_tiles;
-        tc_grid_barrier(p.ctrl, ++episode * (unsigned long long)G);
+        // keys of this CTA are out: count it.  Only the owners wait for all G counts; everybody else goes on to the barrier.
+        __syncthreads();
+        if (tid == 0) red_add_release_u64(p.ctrl + 16, 1ull);
 
         // ================= owners: Eq. 10, Eq. 11, Eq. 18, per-signal stop test ==================================================
-        for (int b = blockIdx.x; b < p.B; b += G) {
-            if (!p.state[b].active) continue;
-            const unsigned long long key = ld_relaxed_u64(p.keys + (t % 3) * 64 + b);
+        if (owner && my_active) {
+            if (tid == 0) while (ld_acquire_u64(p.ctrl + 16) < (unsigned long long)(t + 1) * (unsigned long long)G) {}
+            __syncthreads();
+            TC_STAMP(tid == 0, 6);
+            const unsigned long long key = ld_relaxed_u64(p.keys + (t % 3) * 64 + b_own);
             const int i = key_index(key);
             const float c = key_value(key);
             const double cd = (double)c;
             const float* psi_i = p.psi_t + (int64_t)i * p.ld;
             double s2 = 0.0;
-            for (int n = tid; n < p.N; n += kTcThreads) {
-                const double v = p.r64[(size_t)b * p.Nr + n] - cd * (double)__ldg(psi_i + n);
-                tc_publish(p, b, n, v);
-                s2 += v * v;
+            if (reg_r) {
+                float pv[kTcRegElems];
+#pragma unroll
+                for (int k = 0; k < kTcRegElems; k++) {
+                    const int n = tid + k * kTcThreads;
+                    pv[k] = n < p.N ? __ldg(psi_i + n) : 0.f;
+                }
+#pragma unroll
+                for (int k = 0; k < kTcRegElems; k++) {
+                    const int n = tid + k * kTcThreads;
+                    if (n < p.N) {
+                        const double v = rreg[k] - cd * (double)pv[k];
+                        rreg[k] = v;
+                        tc_publish(p, b_own, n, v);
+                        s2 += v * v;
+                    }
+                }
+            } else {
+                for (int n = tid; n < p.N; n += kTcThreads) {
+                    const double v = p.r64[(size_t)b_own * p.Nr + n] - cd * (double)__ldg(psi_i + n);
+                    p.r64[(size_t)b_own * p.Nr + n] = v;
+                    tc_publish(p, b_own, n, v);
+                    s2 += v * v;
+                }
             }
+            fence_proxy_async_all();
             const double rr = tc_block_sum(s2, tail->red);
-            const bool done = !(sqrt(rr) > p.state[b].thresh) || (t + 1 >= p.max_iter);
-            if (done)
-                for (int n = tid; n < p.N; n += kTcThreads) p.R[(size_t)b * p.N + n] = (float)p.r64[(size_t)b * p.Nr + n];
-            __syncthreads();                                                    // every thread has read state[b] before it changes
+            const bool done = !(sqrt(rr) > thresh) || (t + 1 >= p.max_iter);
+            if (done) {
+                if (reg_r) {
+#pragma unroll
+                    for (int k = 0; k < kTcRegElems; k++) {
+                        const int n = tid + k * kTcThreads;
+                        if (n < p.N) p.R[(size_t)b_own * p.N + n] = (float)rreg[k];
+                    }
+                } else {
+                    for (int n = tid; n < p.N; n += kTcThreads) p.R[(size_t)b_own * p.N + n] = (float)p.r64[(size_t)b_own * p.Nr + n];
+                }
+            }
             if (tid == 0) {
-                p.x64[(size_t)b * p.M + i] += cd;
-                if (p.idx_trace) p.idx_trace[(size_t)b * p.ldt + t] = i;
-                if (p.c_trace) p.c_trace[(size_t)b * p.ldt + t] = c;
-                st_relaxed_u64(p.keys + ((t + 2) % 3) * 64 + b, 0ull);          // slot of iteration t-1, reused at t+2
+                red_add_f64(p.x64 + (size_t)b_own * p.M + i, cd);              // only this CTA touches row b: plain order of adds
+                if (p.idx_trace) p.idx_trace[(size_t)b_own * p.ldt + t] = i;
+                if (p.c_trace) p.c_trace[(size_t)b_own * p.ldt + t] = c;
+                st_relaxed_u64(p.keys + ((t + 2) % 3) * 64 + b_own, 0ull);      // slot of iteration t-1, reused at t+2
                 if (done) {
-                    p.n_iter[b] = t + 1;
-                    p.state[b].active = 0;
+                    p.n_iter[b_own] = t + 1;
                     atomicAdd(p.ctrl + 5, ~0ull);                               // one signal fewer
                 }
             }
+            my_active = !done;
         }
+        TC_STAMP(tid == 0, 7);
         tc_grid_barrier(p.ctrl, ++episode * (unsigned long long)G);
+        TC_STAMP(tid == 0, 8);
         if (tid == 0) tail->n_active = (int)ld_acquire_u64(p.ctrl + 5);
         __syncthreads();
         n_active = tail->n_active;
@@ -542,7 +625,6 @@ mp_status launch_recover_batched_tc(const BatchedArgs& a, const Workspace& ws, f
     p.psi_t = a.psi_t; p.ld = a.ld; p.Y = a.Y; p.ldy = a.ldy;
     p.X = a.X; p.R = a.R; p.n_iter = a.n_iter; p.idx_trace = a.idx_trace; p.c_trace = a.c_trace; p.ldt = a.ldt;
     p.x64 = ws.x64; p.r64 = ws.r64; p.rs = ws.rs; p.ctrl = ws.ctrl; p.keys = ws.keys;
-    p.state = reinterpret_cast<SigState*>(ws.state);
     p.dbg_C = dbg_C;
     p.N = a.N; p.M = a.M; p.B = a.B; p.Nr = Nr; p.Npad = round_up(a.N, 4);
     p.AT = plan.AT; p.n_tiles = plan.n_tiles; p.n_clusters = plan.n_clusters; p.tiles_per_cluster = plan.tiles_per_cluster;
@@ -559,7 +641,7 @@ mp_status launch_recover_batched_tc(const BatchedArgs& a, const Workspace& ws, f
     at[0].val.clusterDim.x = kTcCluster; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
     at[1].id = cudaLaunchAttributeCooperative;
     at[1].val.cooperative = 1;
-    cfg.attrs = at; cfg.numAttrs = 2;
+    cfg.attrs = at; cfg.numAttrs = options().batched_coop ? 2 : 1;
     cudaError_t e = cudaLaunchKernelEx(&cfg, mp_batched_tc_kernel, tm_psi, tm_rs, p);
     if (e == cudaErrorNotSupported || e == cudaErrorInvalidValue || e == cudaErrorCooperativeLaunchTooLarge) {
         // cluster + cooperative attribute refused: the grid is sized from cudaOccupancyMaxActiveClusters, so all
@@ -570,7 +652,16 @@ mp_status launch_recover_batched_tc(const BatchedArgs& a, const Workspace& ws, f
     }
     if (e != cudaSuccess) return cuda_fail(e, "cudaLaunchKernelEx(mp_batched_tc_kernel)");
     count_launch();
+    options().info_tc_clusters = plan.n_clusters; options().info_tc_at = plan.AT; options().info_tc_stages = plan.S;
     return MP_OK;
 }
 
 }  // namespace mp
+
+#ifdef MP_TC_TIMING
+extern "C" __attribute__((visibility("default"))) int mp_debug_tc_stamps(unsigned long long* out, size_t bytes)
+{
+    if (bytes > sizeof(mp::g_tc_stamps)) bytes = sizeof(mp::g_tc_stamps);
+    return (int)cudaMemcpyFromSymbol(out, mp::g_tc_stamps, bytes);
+}
+#endif

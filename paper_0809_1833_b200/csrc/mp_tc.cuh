@@ -74,6 +74,25 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, float (&v)[16])
     for (int i = 0; i < 16; i++) v[i] = __uint_as_float(r[i]);
 }
 
+// the same load without the wait, so that several can be in flight; tmem_ld_wait() makes all of them readable
+__device__ __forceinline__ void tmem_ld16_issue(uint32_t taddr, uint32_t (&r)[16])
+{
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+          "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+        : "r"(taddr)
+        : "memory");
+}
+__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+// ties the registers of an issued load to a point after tmem_ld_wait() so that no use is scheduled before it
+__device__ __forceinline__ void tmem_ld_pin(uint32_t (&r)[16])
+{
+    asm volatile("" : "+r"(r[0]), "+r"(r[1]), "+r"(r[2]), "+r"(r[3]), "+r"(r[4]), "+r"(r[5]), "+r"(r[6]), "+r"(r[7]),
+                      "+r"(r[8]), "+r"(r[9]), "+r"(r[10]), "+r"(r[11]), "+r"(r[12]), "+r"(r[13]), "+r"(r[14]), "+r"(r[15])
+                 :: "memory");
+}
+
 // Shared-memory matrix descriptor: K-major operand, 128-byte swizzle, rows of 128 bytes (32 fp32), 8-row groups
 // 1024 bytes apart (the layout a 2-D TMA box {32 floats, rows} with SWIZZLE_128B produces).  Tile base 1024-B aligned.
 // Field positions: start address [0,14) >>4, leading byte offset [16,30) (unused for swizzled K-major), stride byte
@@ -112,6 +131,14 @@ __device__ __forceinline__ float ld_dsmem_f32(uint32_t cluster_addr)
 {
     float v;
     asm volatile("ld.shared::cluster.f32 %0, [%1];" : "=f"(v) : "r"(cluster_addr) : "memory");
+    return v;
+}
+// the same load without the "memory" clobber: it stays ordered after the preceding volatile asm (the cluster-scope
+// acquire wait) but is no compiler barrier, so a batch of independent loads is issued back to back
+__device__ __forceinline__ float ld_dsmem_f32_nv(uint32_t cluster_addr)
+{
+    float v;
+    asm volatile("ld.shared::cluster.f32 %0, [%1];" : "=f"(v) : "r"(cluster_addr));
     return v;
 }
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr)
