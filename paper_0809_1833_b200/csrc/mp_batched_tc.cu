@@ -6,16 +6,16 @@
 //   * grid = clusters of 4 CTAs, all co-resident.  A cluster owns tiles of AT <= 256 consecutive atoms; inside the
 //     cluster the reduction dimension N is split four ways (split-K), CTA rank q takes k-chunks [q nc/4, (q+1) nc/4).
 //   * per k-chunk of 32 floats one pipeline stage holds the dictionary tile (AT x 32, TMA, 128-byte swizzle, K-major)
-//     and the residual tile (128 x 32: rows 0-63 = tf32-exact high parts of the 64 residuals, rows 64-127 = the
-//     low parts r - hi).  Worker warps derive the low part of the dictionary tile (psi - tf32(psi), exact) into a
+//     and the residual tile (128 x 32: row 2b = tf32-exact high part of residual b, row 2b+1 = its
+//     low part r - hi).  Worker warps derive the low part of the dictionary tile (psi - tf32(psi), exact) into a
 //     second buffer.  The MMA warp then issues, per 8 floats of k,
 //         D_hi[128 x AT] += [R_hi; R_lo] . Psi_hi^T     and     D_lo[128 x AT] += [R_hi; R_lo] . Psi_lo^T
-//     so rows b and 64+b of the two accumulators together hold all four partial products of
+//     so rows 2b and 2b+1 of the two accumulators together hold all four partial products of
 //     (R_hi + R_lo)(Psi_hi + Psi_lo): an UMMA with M = 64 costs the same tensor time as M = 128, so the low-part rows
 //     ride along for free.  The tensor core truncates its fp32 accumulator on every accumulation (measured: a
 //     coherent sum loses about 2^-24.2 relative per UMMA), so the small Psi_lo products get their own accumulator
 //     instead of costing the large one a second truncation per k-step; split-K keeps each chain N/32 UMMAs long.
-//   * epilogue: TMEM -> registers, rows b and 64+b added, the four split-K partials are exchanged through
+//   * epilogue: TMEM -> registers, rows 2b and 2b+1 added (one shuffle), the four split-K partials are exchanged through
 //     distributed shared memory and added in rank order (deterministic), CTA q takes a quarter of the tile's atoms,
 //     per-signal packed (|c|, index, sign) argmax (Eq. 16, lowest index on ties) -> red.max.u64 -> grid barrier.
 //   * signal b is owned by CTA b: it applies r_b <- r_b - c psi_i (Eq. 11) to the float64 residual, recomputes
@@ -61,7 +61,7 @@ struct BatchedTcParams {
     const float* psi_t; int64_t ld;
     const float* Y; int64_t ldy;
     float* X; float* R; int* n_iter; int* idx_trace; float* c_trace; int64_t ldt;
-    double* x64; double* r64; float* rs;            // rs: [128][Nr]  rows 0-63 hi parts, rows 64-127 lo parts
+    double* x64; double* r64; float* rs;            // rs: [128][Nr]  row 2b = hi part of r_b, row 2b+1 = lo part
     unsigned long long* ctrl;                       // [0] grid-barrier counter, [5] number of active signals, [16] CTAs whose keys are out
     unsigned long long* keys;                       // [3][64] rotating per-signal argmax keys
     float* dbg_C;                                   // nullable: B x M correlations of iteration 0 (mp_correlate_batched)
@@ -72,7 +72,7 @@ struct BatchedTcParams {
 
 struct TcTail {
     uint64_t full[kTcMaxStages], empty[kTcMaxStages], lo_full[2], lo_empty[2], tmem_full, tmem_empty, cl_ready, cl_done;
-    unsigned long long skeys[4 * 64];
+    unsigned long long skeys[8 * 64];
     double red[16];
     uint32_t tmem_base;
     int n_active;
@@ -116,13 +116,13 @@ __device__ __forceinline__ double tc_block_sum(double v, double* red)
     return s;
 }
 
-// publishes the hi / lo split of the fp32 rounding of one residual element (the tensor-core A operand rows b, 64+b)
+// publishes the hi / lo split of the fp32 rounding of one residual element (the tensor-core A operand rows 2b, 2b+1)
 __device__ __forceinline__ void tc_publish(const BatchedTcParams& p, int b, int n, double v)
 {
     const float f = (float)v;
     const float hi = tf32_rn(f);
-    p.rs[(size_t)b * p.Nr + n] = hi;
-    p.rs[(size_t)(64 + b) * p.Nr + n] = tf32_rn(f - hi);
+    p.rs[(size_t)(2 * b) * p.Nr + n] = hi;
+    p.rs[(size_t)(2 * b + 1) * p.Nr + n] = tf32_rn(f - hi);
 }
 
 __global__ void __launch_bounds__(kTcThreads, 1)
@@ -292,8 +292,8 @@ mp_batched_tc_kernel(const __grid_constant__ CUtensorMap tm_psi, const __grid_co
             // ================= workers: dictionary low parts, then the epilogue =========================================
             const int wtid = tid - 64;
             const int q4 = warp & 3, half = (warp - 2) >> 2;
-            const int L = q4 * 32 + lane, b_row = L & 63;
-            unsigned long long best = 0ull;
+            const int b_row = q4 * 16 + (lane >> 1);                           // TMEM lane 2b = hi row of signal b, 2b+1 = lo row
+            unsigned long long best4[4] = {0ull, 0ull, 0ull, 0ull};
             for (int j = 0; j < n_my_tiles; j++) {
                 const int tile = cl + j * p.n_clusters;
                 for (int c = 0; c < my_nc; c++, g_wrk++) {
@@ -312,33 +312,27 @@ mp_batched_tc_kernel(const __grid_constant__ CUtensorMap tm_psi, const __grid_co
                     if (lane == 0) mbar_arrive(&tail->lo_full[h]);
                 }
                 TC_STAMP(wtid == 0, 1);
-                // ---- epilogue of this tile: D rows b (hi residual part) + 64+b (lo residual part) -> P[col][b] -----------
+                // ---- epilogue of this tile: D rows 2b (hi residual part) + 2b+1 (lo residual part) -> P[col][b] -----------
                 const unsigned int ph = (tile_count + j) & 1;
                 mbar_wait(&tail->tmem_full, ph);
                 TC_STAMP(wtid == 0, 2);
                 tc_fence_after_sync();
                 const int col0 = half * (p.AT >> 1), col1 = col0 + (p.AT >> 1);
                 const uint32_t trow = tmem + ((uint32_t)(q4 * 32) << 16);
-                if (L >= 64) {
-                    for (int col = col0; col < col1; col += 16) {
-                        uint32_t v[16], w[16];
-                        tmem_ld16_issue(trow + (uint32_t)col, v);
-                        tmem_ld16_issue(trow + 256u + (uint32_t)col, w);
-                        tmem_ld_wait(); tmem_ld_pin(v); tmem_ld_pin(w);
+                for (int col = col0; col < col1; col += 16) {
+                    uint32_t v[16], w[16];
+                    tmem_ld16_issue(trow + (uint32_t)col, v);
+                    tmem_ld16_issue(trow + 256u + (uint32_t)col, w);
+                    tmem_ld_wait(); tmem_ld_pin(v); tmem_ld_pin(w);
+                    float sum[16];
 #pragma unroll
-                        for (int i = 0; i < 16; i++) P[(col + i) * 64 + b_row] = __uint_as_float(v[i]) + __uint_as_float(w[i]);
+                    for (int i = 0; i < 16; i++) {
+                        const float a = __uint_as_float(v[i]) + __uint_as_float(w[i]);
+                        sum[i] = a + __shfl_xor_sync(0xffffffffu, a, 1);        // hi-row + lo-row of the signal, same bits in both lanes
                     }
-                }
-                named_bar_sync(1, kTcWorkers);
-                if (L < 64) {
-                    for (int col = col0; col < col1; col += 16) {
-                        uint32_t v[16], w[16];
-                        tmem_ld16_issue(trow + (uint32_t)col, v);
-                        tmem_ld16_issue(trow + 256u + (uint32_t)col, w);
-                        tmem_ld_wait(); tmem_ld_pin(v); tmem_ld_pin(w);
+                    const int i0 = (lane & 1) * 8;                              // the pair shares the 16 stores
 #pragma unroll
-                        for (int i = 0; i < 16; i++) P[(col + i) * 64 + b_row] += __uint_as_float(v[i]) + __uint_as_float(w[i]);
-                    }
+                    for (int i = 0; i < 8; i++) P[(col + i0 + i) * 64 + b_row] = (lane & 1) ? sum[8 + i] : sum[i];
                 }
                 tc_fence_before_sync();
                 __syncwarp();
@@ -350,34 +344,39 @@ mp_batched_tc_kernel(const __grid_constant__ CUtensorMap tm_psi, const __grid_co
                 mbar_wait_cluster(&tail->cl_ready, ph);
                 TC_STAMP(wtid == 0, 4);
                 {
-                    const int b = wtid & 63, g4 = wtid >> 6;
-                    const int per_cta = p.AT >> 2, per_grp = p.AT >> 4;
-                    const int jc0 = (int)q * per_cta + g4 * per_grp;
+                    // CTA q reduces columns [q AT/4, (q+1) AT/4); a thread takes 4 signals (one 128-bit DSMEM load per rank)
+                    const int b4 = (wtid & 15) * 4, colsub = wtid >> 4;
+                    const int per_cta = p.AT >> 2;
+                    const int jc_begin = (int)q * per_cta + colsub, jc_end = ((int)q + 1) * per_cta;
                     const uint32_t p_addr = smem_u32(P);
                     uint32_t pr[kTcCluster];
 #pragma unroll
                     for (uint32_t r = 0; r < kTcCluster; r++) pr[r] = map_to_cta(p_addr, r);
-                    for (int jb = jc0; jb < jc0 + per_grp; jb += 8) {          // per_grp = AT/16 is 2, 4, 6, ... : batches of <= 8
-                        const int nb = min(8, jc0 + per_grp - jb);
-                        float part[kTcCluster][8];
+                    float4 part[4][kTcCluster];
 #pragma unroll
-                        for (int u = 0; u < 8; u++) {
-                            if (u < nb) {
-                                const uint32_t off = (uint32_t)((jb + u) * 64 + b) * 4u;
+                    for (int u = 0; u < 4; u++) {
+                        const int jc = jc_begin + 16 * u;
+                        if (jc < jc_end) {
+                            const uint32_t off = (uint32_t)(jc * 64 + b4) * 4u;
 #pragma unroll
-                                for (int r = 0; r < kTcCluster; r++) part[r][u] = ld_dsmem_f32_nv(pr[r] + off);
-                            }
+                            for (int r = 0; r < kTcCluster; r++) part[u][r] = ld_dsmem_f32x4_nv(pr[r] + off);
                         }
+                    }
 #pragma unroll
-                        for (int u = 0; u < 8; u++) {
-                            if (u < nb) {
-                                const float v = ((part[0][u] + part[1][u]) + part[2][u]) + part[3][u];   // rank order: deterministic
-                                const int atom = tile * p.AT + jb + u;
-                                if (atom < p.M && b < p.B) {
-                                    const unsigned long long k = pack_key(v, atom);
-                                    best = k > best ? k : best;
-                                    if (p.dbg_C && t == 0) p.dbg_C[(size_t)b * p.M + atom] = v;
-                                }
+                    for (int u = 0; u < 4; u++) {
+                        const int jc = jc_begin + 16 * u;
+                        const int atom = tile * p.AT + jc;
+                        if (jc < jc_end && atom < p.M) {
+                            float v[4];                                         // rank order: deterministic
+                            v[0] = ((part[u][0].x + part[u][1].x) + part[u][2].x) + part[u][3].x;
+                            v[1] = ((part[u][0].y + part[u][1].y) + part[u][2].y) + part[u][3].y;
+                            v[2] = ((part[u][0].z + part[u][1].z) + part[u][2].z) + part[u][3].z;
+                            v[3] = ((part[u][0].w + part[u][1].w) + part[u][2].w) + part[u][3].w;
+#pragma unroll
+                            for (int e = 0; e < 4; e++) {
+                                const unsigned long long k = pack_key(v[e], atom);
+                                best4[e] = k > best4[e] ? k : best4[e];
+                                if (p.dbg_C && t == 0 && b4 + e < p.B) p.dbg_C[(size_t)(b4 + e) * p.M + atom] = v[e];
                             }
                         }
                     }
@@ -389,13 +388,21 @@ mp_batched_tc_kernel(const __grid_constant__ CUtensorMap tm_psi, const __grid_co
                 }
             }
             // ---- per-signal argmax of this CTA -> grid-wide key slot of iteration t --------------------------------------------
-            tail->skeys[wtid] = best;
+#pragma unroll
+            for (int e = 0; e < 4; e++) {                                      // lanes l and l+16 hold the same four signals
+                const unsigned long long o = __shfl_xor_sync(0xffffffffu, best4[e], 16);
+                best4[e] = o > best4[e] ? o : best4[e];
+            }
+            if (lane < 16) {
+#pragma unroll
+                for (int e = 0; e < 4; e++) tail->skeys[(warp - 2) * 64 + lane * 4 + e] = best4[e];
+            }
             named_bar_sync(1, kTcWorkers);
             TC_STAMP(wtid == 0, 5);
             if (wtid < 64 && wtid < p.B && n_my_tiles > 0) {
                 unsigned long long k = tail->skeys[wtid];
 #pragma unroll
-                for (int g4 = 1; g4 < 4; g4++) { const unsigned long long o = tail->skeys[g4 * 64 + wtid]; k = o > k ? o : k; }
+                for (int w8 = 1; w8 < 8; w8++) { const unsigned long long o = tail->skeys[w8 * 64 + wtid]; k = o > k ? o : k; }
                 if (k) red_max_u64(p.keys + (t % 3) * 64 + wtid, k);
             }
         }
