@@ -46,6 +46,20 @@ def load_peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
+def load_tf32_peak():
+    """Dense TF32 tensor peak in TFLOP/s: the measured sustained bf16 cuBLAS figure (the batched kernel is timed inside
+    a long step) x the guide's nominal tf32/bf16 ratio 1.1/2.25."""
+    ratio = 1.1 / 2.25
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            d = json.load(open(p))
+            return float(d["bf16_tflops_sustained"]) * ratio, "measured bf16_tflops_sustained x 1.1/2.25 (nominal tf32/bf16)"
+        except Exception:
+            pass
+    return 1400.0 * ratio, "fallback (B200_PROFILING.md 1.4 PFLOP/s sustained bf16) x 1.1/2.25"
+
+
 def ncu_traffic_per_iteration():
     """DRAM bytes per MP iteration of the dominant kernel from the committed ncu capture, or None."""
     p = os.path.join(ROOT, "profiles", "dominant_kernel_traffic.txt")
@@ -153,7 +167,7 @@ def aggregate(dist, elapsed_local, units_local, device):
 
 
 def workload_name(cfg):
-    return (f"{cfg.name}: single-signal MP fp32, N={cfg.N}, M={cfg.M}, K={cfg.K}, {cfg.dictionary} dictionary, "
+    return (f"{cfg.name}: {'single-signal' if cfg.B == 1 else 'batched'} MP fp32, N={cfg.N}, M={cfg.M}, K={cfg.K}, {cfg.dictionary} dictionary, "
             f"eps={cfg.eps:g}, max_iter={cfg.max_iter}" + (f", B={cfg.B}" if cfg.B > 1 else ""))
 
 
@@ -263,13 +277,26 @@ def main():
 
     # ---- roofline of the dominant kernel (the persistent MP loop; one launch per solve) -------------------------
     peak, peak_src = load_peaks()
+    solve_ms = float(np.mean(ms_solve))
+    if B > 1 and mp.mp_get_int("info_tc_clusters"):
+        # batched path: the contraction Psi^T R on the tensor cores.  Algorithmic flops per lock-step iteration =
+        # 3 x 2NMB (three TF32 products per fp32-accurate product); the dictionary is L2-resident (64 MiB).
+        tpeak, tsrc = load_tf32_peak()
+        alg_flops = its_max * 3.0 * 2.0 * N * M * B
+        ach = alg_flops / (solve_ms * 1e-3) / 1e12
+        roofline = {"bound": "tensor", "achieved": ach, "peak": tpeak, "unit": "TFLOP/s", "frac": ach / tpeak, "traffic": None,
+                    "peak_source": tsrc, "kernel": mp_kernel_name(mp), "algorithmic_flops_per_launch": alg_flops,
+                    "kernel_ms": solve_ms, "us_per_lockstep_iteration": 1e3 * solve_ms / max(its_max, 1),
+                    "lockstep_iterations": its_max,
+                    "note": "measured limiter is shared-memory bandwidth (M = 128 rows per UMMA) and the per-iteration "
+                            "argmax/update/barrier chain, see profiles/batched_r01.md"}
     # algorithmic bytes per launch: each iteration streams the dictionary once (4NM) and re-reads the winning atom (4N)
     # (SURVEY.md 8(d)); the batched loop runs until its slowest signal stops.
     alg_bytes = its_max * (4.0 * N * M + 4.0 * N * B)
-    solve_ms = float(np.mean(ms_solve))
     achieved = alg_bytes / (solve_ms * 1e-3) / 1e9
     per_it = ncu_traffic_per_iteration() if args.config == "cfg3" else None
-    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+    if not (B > 1 and mp.mp_get_int("info_tc_clusters")):
+      roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": per_it * its_max if per_it else None, "peak_source": peak_src,
                 "kernel": mp_kernel_name(mp), "algorithmic_bytes_per_launch": alg_bytes, "kernel_ms": solve_ms,
                 "us_per_iteration": 1e3 * solve_ms / max(its_max, 1)}
@@ -291,6 +318,21 @@ def main():
                "ms_per_step": 1e3 * dt_max / args.steps,
                "note": "mp_recover_host: cudaMalloc + H2D(Psi, y) + normalise + solve + D2H(x, r, n_iter) + free per step"}
 
+    if not args.no_e2e and B > 1:
+        hp = torch.from_numpy(psi_raw).pin_memory(); hY = torch.from_numpy(Y).pin_memory()
+        for _ in range(2):
+            mp.mp_recover_batched_host(hp, hY, cfg.eps, cfg.max_iter, normalize=True, device=local)
+        if dist: dist.barrier()
+        t0 = time.perf_counter(); its = 0
+        for _ in range(args.steps):
+            its += int(mp.mp_recover_batched_host(hp, hY, cfg.eps, cfg.max_iter, normalize=True, device=local).n_iter.sum().item())
+        dt = time.perf_counter() - t0
+        dt_max, its_e = aggregate(dist, dt, float(its), dev)
+        e2e = {"value": its_e / dt_max, "unit": UNIT,
+               "h2d_bytes_per_step": 4 * N * M + 4 * N * B, "d2h_bytes_per_step": 4 * M * B + 4 * N * B + 4 * B,
+               "ms_per_step": 1e3 * dt_max / args.steps,
+               "note": "mp_recover_batched_host: cudaMalloc + H2D(Psi, Y) + normalise + solve + D2H(X, R, n_iter) + free per step"}
+
     if rank == 0:
         cb = None
         if not args.no_cpu_baseline and world == 1:
@@ -300,7 +342,7 @@ def main():
             "ms_per_step": ms_total_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": workload_name(cfg), "iterations_per_step": its_per_step,
-                       "step": "mp_normalize_columns + mp_recover (whole solve to the eps stop)",
+                       "step": "mp_normalize_columns + %s (whole solve to the eps stop)" % ("mp_recover" if B == 1 else "mp_recover_batched"),
                        "l2": "dictionary 4NM = %.0f MiB > 126 MB L2: inputs larger than L2, no flush" % (4.0 * N * M / 2**20)
                              if 4.0 * N * M > 126e6 else "dictionary fits in L2 (cache-resident regime, by design of this config)",
                        "parallelism": "replicas only" if world > 1 else "1 GPU"},

@@ -27,6 +27,13 @@ import oracle
 
 GAP_TOL = 1e-4      # north_star: "top-two |c| gap exceeds 1e-4 relative"
 C_TOL = 4e-6        # |c_gpu - c_ref| / ||r_t||, see DESIGN.md "Tolerances"
+
+
+def c_tol_tensor_core(N: int) -> float:
+    """Step-value tolerance of the batched tensor-core path: the tcgen05 fp32 accumulator is
+    truncated (not rounded) on every UMMA, at most one ulp = 2^-23 of the running sum (|running sum| <= ||r||), and
+    each split-K accumulator chain is N/32 UMMAs long; measured bias is about 0.37 of this bound."""
+    return C_TOL + (N / 32.0) * 2.0 ** -23
 NORM_TOL = 1e-4     # north_star: final ||r|| within 1e-4 relative
 X_TOL = 1e-4        # north_star: ||x_gpu - x_ref|| / ||x_ref||
 
@@ -46,7 +53,7 @@ class Grade:
 
 def grade_single(psi32: np.ndarray, y32: np.ndarray, eps: float, max_iter: int,
                  x_gpu, r_gpu, n_iter_gpu, idx_gpu, c_gpu, *, x_true=None, support=None,
-                 nthreads: int | None = None, ref: "oracle.MPResult | None" = None) -> Grade:
+                 nthreads: int | None = None, ref: "oracle.MPResult | None" = None, c_tol: float = C_TOL) -> Grade:
     nthreads = nthreads or oracle.default_threads()
     eps = float(np.float32(eps))                       # the very float the GPU received
     y = y32.astype(np.float64)
@@ -93,7 +100,7 @@ def grade_single(psi32: np.ndarray, y32: np.ndarray, eps: float, max_iter: int,
         f"vs oracle idx {rp.argmax_ref[bad[0]]} max={rp.cmax_ref[bad[0]]:.9e} gap={rp.gap[bad[0]]:.3e}")
     c_err = np.abs(c_gpu - rp.c_at_idx) / np.maximum(rp.rnorm[:t_gpu], np.finfo(np.float64).tiny) if t_gpu else np.zeros(0)
     max_c_err = float(c_err.max()) if t_gpu else 0.0
-    assert max_c_err <= C_TOL, f"step value error {max_c_err:.3e} ||r|| at t={int(c_err.argmax())} exceeds {C_TOL}"
+    assert max_c_err <= c_tol, f"step value error {max_c_err:.3e} ||r|| at t={int(c_err.argmax())} exceeds {c_tol}"
 
     # ---- G4 final residual and coefficients ---------------------------------------------------------------------
     nr_gpu = float(np.linalg.norm(r_gpu))
@@ -149,7 +156,7 @@ def residual_at(psi32: np.ndarray, y32: np.ndarray, idx, c, t: int) -> np.ndarra
     return r
 
 
-def grade_sampled(psi32, y32, idx_gpu, c_gpu, n_iter_gpu, r_gpu, sample_ts, nthreads=None):
+def grade_sampled(psi32, y32, idx_gpu, c_gpu, n_iter_gpu, r_gpu, sample_ts, nthreads=None, c_tol: float = C_TOL):
     """Full-size check on SAMPLED iterations the oracle can compute one by one: for each t in sample_ts the
     state is rebuilt in float64 from the GPU trace, one oracle correlation pass gives c_ref, and the GPU's pick
     and step must satisfy G2/G3.  Also checks the final residual (G4)."""
@@ -168,7 +175,7 @@ def grade_sampled(psi32, y32, idx_gpu, c_gpu, n_iter_gpu, r_gpu, sample_ts, nthr
         i = int(idx_gpu[t])
         assert i == i_ref or (gap <= GAP_TOL and a[i] >= (1 - GAP_TOL) * a1), f"illegal pick at sampled t={t}"
         err = abs(float(c_gpu[t]) - c[i]) / oracle.nrm2(r)
-        assert err <= C_TOL, f"step value error {err:.3e} at sampled t={t}"
+        assert err <= c_tol, f"step value error {err:.3e} at sampled t={t}"
         out.append((t, gap, err))
     r_fin = residual_at(psi32, y32, idx_gpu, c_gpu, t_gpu)
     nr = oracle.nrm2(r_fin)

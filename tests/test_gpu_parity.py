@@ -279,14 +279,51 @@ def test_batched_every_signal_graded_like_a_single_run(mp, B, N, M, K, algo):
     X, R, T = res.x.cpu().numpy(), res.r.cpu().numpy(), res.n_iter.cpu().numpy()
     I, Cc = res.idx_trace.cpu().numpy(), res.c_trace.cpu().numpy()
     assert T[B // 2] == 0 and not X[B // 2].any() and not R[B // 2].any()
+    c_tol = grading.c_tol_tensor_core(N) if algo == 1 else grading.C_TOL
     for b in range(B):
         t = int(T[b])
         grading.grade_single(pb.psi32, pb.Y[b], cfg.eps, cfg.max_iter, X[b], R[b], t, I[b, :t], Cc[b, :t],
-                             x_true=pb.X[b], support=pb.S[b], nthreads=1)
+                             x_true=pb.X[b], support=pb.S[b], nthreads=1, c_tol=c_tol)
     # and the untraced entry point gives the same bits
     res2 = mp.mp_recover_batched(buf[:, :N], Yb[:, :N], cfg.eps, cfg.max_iter)
     torch.cuda.synchronize()
     assert torch.equal(res2.x, res.x) and torch.equal(res2.r, res.r) and torch.equal(res2.n_iter, res.n_iter)
+
+
+def test_cfg5_full_size_batched_grading(mp):
+    """CFG5 (B=64 signals, N=2048, M=8192) in the launch configuration bench.py times (batched_algo auto = the lock-step
+    tensor-core kernel): four signals get the full teacher-forced grading, every signal gets sampled iterations rebuilt
+    in float64 from its trace, its final residual, its support and its coefficients checked."""
+    pb = problems.make_problem(synth.config("cfg5"), 1)
+    c = pb.cfg
+    mp.mp_set_int("batched_algo", 0)
+    res = mp.mp_recover_batched(dev(pb.psi32), dev(pb.Y), c.eps, c.max_iter, trace=True)
+    torch.cuda.synchronize()
+    assert mp.mp_get_int("info_tc_clusters") > 0, "cfg5 must run on the tensor-core kernel"
+    X, R, T = res.x.cpu().numpy(), res.r.cpu().numpy(), res.n_iter.cpu().numpy()
+    I, Cc = res.idx_trace.cpu().numpy(), res.c_trace.cpu().numpy()
+    c_tol = grading.c_tol_tensor_core(c.N)
+    worst = 0.0
+    for b in range(c.B):
+        t = int(T[b])
+        assert 300 < t < 1500
+        if b in (0, 21, 42, 63):
+            g = grading.grade_single(pb.psi32, pb.Y[b], c.eps, c.max_iter, X[b], R[b], t, I[b, :t], Cc[b, :t],
+                                     x_true=pb.X[b], support=pb.S[b], c_tol=c_tol)
+            assert g.exact_recovery
+            worst = max(worst, g.max_c_err)
+        else:
+            ts = sorted(set([0, 1, t // 3, (2 * t) // 3, t - 2, t - 1]))
+            out = grading.grade_sampled(pb.psi32, pb.Y[b], I[b], Cc[b], t, R[b], ts, c_tol=c_tol)
+            worst = max(worst, max(e for _, _, e in out))
+        sel, sup = set(I[b, :t].tolist()), set(pb.S[b].tolist())
+        assert sel <= sup                                                    # never an off-support atom (SURVEY B.5)
+        tau = 1e-3 * np.max(np.abs(pb.X[b]))                                 # reading R13: entries below 2 tau are "don't care"
+        assert all(abs(pb.X[b][m]) < 2 * tau for m in sup - sel)
+        assert np.linalg.norm(X[b] - pb.X[b]) <= 1e-4 * np.linalg.norm(pb.X[b])
+        ny = np.linalg.norm(pb.Y[b].astype(np.float64))
+        assert np.linalg.norm(R[b].astype(np.float64)) <= np.float32(c.eps) * ny * (1 + 1e-6)
+    print(f"cfg5 worst step-value error {worst:.3e} ||r|| (tolerance {c_tol:.3e})")
 
 
 # ------------------------------------------------------------------------------------------ host-buffer entry points (e2e path)
