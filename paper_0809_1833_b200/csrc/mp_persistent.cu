@@ -349,9 +349,30 @@ static bool make_plan(int N, int M, const DeviceInfo& di, PersistentPlan* plan)
         D = (int)o.depth;
         W = max_slots / D;
     } else {
-        D = 1;
-        W = max_slots;
-        if (W > kMaxWarps) { W = 16; D = max_slots / W; }
+        // Choose the warp count for BALANCE.  The CTA with the most atoms sets the iteration time, and a warp works
+        // through its groups one after another, so what counts is rounds = ceil(groups / W): with 111 atoms, 22 warps
+        // need 6 rounds of which the last is 16 % full (measured 47.9 us per iteration at CFG3), 16 warps need 7 full
+        // rounds (43.6 us).  Score = fill of the rounds, scaled down if fewer than 96 KB can be in flight (HBM latency x
+        // per-SM bandwidth share is about 88 KB); a share that fits entirely in the slots (stationary dictionary)
+        // beats everything.  Ties go to more warps.
+        const int G = di.sm_count > 0 ? di.sm_count : 1;
+        const int atoms_max = (M + G - 1) / G;
+        const int groups = (atoms_max + A - 1) / A;
+        double best_score = -1.0;
+        W = 1; D = 1;
+        for (int w = 1; w <= kMaxWarps; w++) {
+            int d = max_slots / w;
+            if (d < 1) break;
+            if (w < 8 && max_slots >= 8 && groups > w) continue;              // fewer than 8 warps cannot keep up with the stream
+            if (d > 64) d = 64;
+            const int per_warp_items = ((groups + w - 1) / w) * KC;
+            const bool fits = per_warp_items <= d;
+            const double fill = (double)groups / ((double)((groups + w - 1) / w) * w);
+            const double inflight = (double)w * (double)(d < per_warp_items ? d : per_warp_items) * slot_bytes;
+            double score = fill * (inflight >= 96.0 * 1024 ? 1.0 : inflight / (96.0 * 1024));
+            if (fits) score = 10.0 + fill;
+            if (score >= best_score) { best_score = score; W = w; D = d; }
+        }
     }
     if (W > kMaxWarps) W = kMaxWarps;
     if (W < 1 || D < 1) return false;
@@ -362,7 +383,6 @@ static bool make_plan(int N, int M, const DeviceInfo& di, PersistentPlan* plan)
     plan->grid = o.grid > 0 ? (int)o.grid : di.sm_count;
     if (plan->grid > di.sm_count) plan->grid = di.sm_count;
     plan->smem = fixed + (size_t)W * D * (slot_bytes + 8);
-    (void)M;
     return true;
 }
 
