@@ -123,8 +123,10 @@ MP_API mp_status mp_correlate_batched(const float* psi_t, int N, int M, int64_t 
 MP_API const char* mp_last_error(void);
 
 /* Tuning / diagnostic knobs (process-wide, not part of the method).  Unknown name -> MP_ERR_INVALID_ARG.
- *   "algo"          0 = auto (default), 1 = persistent cooperative kernel, 2 = stream loop of small kernels
- *                   (general fallback; synchronises the host every "chunk" iterations to read the stop flag)
+ *   "algo"          0 = auto (default: 3 if it fits, else 1, else 2), 1 = persistent cooperative kernel fed by TMA bulk
+ *                   copies through shared memory, 2 = stream loop of small kernels (general fallback; synchronises the
+ *                   host every "chunk" iterations to read the stop flag), 3 = persistent cooperative kernel that streams
+ *                   the dictionary into registers with 128-bit loads
  *   "warps"         consumer warps per CTA of the persistent kernel (0 = auto)
  *   "slot_bytes"    bytes of one shared-memory stage (0 = auto);   "depth"  stages per warp (0 = auto)
  *   "grid"          CTAs of the persistent kernel (0 = auto = one per SM)

@@ -185,6 +185,8 @@ mp_status mp_recover(const float* psi_t, int N, int M, int64_t ld,
     const int64_t algo = options().algo;
     if (algo == 2) return launch_recover_streamloop(a, ws, s);
     if (algo == 1) return launch_recover_persistent(a, ws, s);
+    if (algo == 3) return launch_recover_persistent_ldg(a, ws, s);
+    if (persistent_ldg_supported(N, M)) return launch_recover_persistent_ldg(a, ws, s);
     if (persistent_supported(N, M)) return launch_recover_persistent(a, ws, s);
     return launch_recover_streamloop(a, ws, s);
 }

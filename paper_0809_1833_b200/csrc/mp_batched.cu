@@ -16,9 +16,10 @@ static mp_status launch_batched_sequential(const BatchedArgs& a, const Workspace
                       a.X + (int64_t)b * a.M, a.R + (int64_t)b * a.N, a.n_iter + b,
                       a.idx_trace ? a.idx_trace + (int64_t)b * a.ldt : nullptr,
                       a.c_trace ? a.c_trace + (int64_t)b * a.ldt : nullptr};
-        mp_status st = (options().algo != 2 && persistent_supported(a.N, a.M))
-                           ? launch_recover_persistent(s, one, stream)
-                           : launch_recover_streamloop(s, one, stream);
+        const int64_t algo = options().algo;
+        mp_status st = (algo != 2 && algo != 1 && persistent_ldg_supported(a.N, a.M)) ? launch_recover_persistent_ldg(s, one, stream)
+                       : (algo != 2 && persistent_supported(a.N, a.M))                 ? launch_recover_persistent(s, one, stream)
+                                                                                       : launch_recover_streamloop(s, one, stream);
         if (st != MP_OK) return st;
     }
     return MP_OK;

@@ -57,6 +57,8 @@ struct RecoverArgs {
 };
 mp_status launch_recover_persistent(const RecoverArgs& a, const Workspace& ws, cudaStream_t stream);
 bool persistent_supported(int N, int M);
+mp_status launch_recover_persistent_ldg(const RecoverArgs& a, const Workspace& ws, cudaStream_t stream);
+bool persistent_ldg_supported(int N, int M);
 mp_status launch_recover_streamloop(const RecoverArgs& a, const Workspace& ws, cudaStream_t stream);
 
 struct BatchedArgs {

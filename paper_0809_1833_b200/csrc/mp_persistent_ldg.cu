@@ -1,0 +1,316 @@
+// mp_persistent_ldg.cu -- "algo 3": the whole MP loop (Eq. 8-12) as one persistent cooperative kernel whose
+// correlation pass reads the dictionary straight from global memory into registers (128-bit ld.global.cg, many in
+// flight per lane) instead of staging it in shared memory with TMA bulk copies (algo 1, mp_persistent.cu).
+//
+// Why a second streaming scheme: measured on B200, the TMA-fed kernels top out near 6.5 TB/s chip-wide whether the
+// dictionary comes from HBM or from L2, while plain 128-bit loads reach 7.3 TB/s from HBM and 17-18 TB/s from L2
+// (profiles/persistent_r01.md).  So this variant is what the cache-resident regime (CFG2, CFG4 <= 64 MiB) wants, and
+// it removes the shared-memory staging traffic altogether: shared memory only holds the residual.
+//
+//   * grid = one CTA per SM (cooperative launch); CTA b owns atoms [b*M/G, (b+1)*M/G).
+//   * work items = (group of A atoms, chunk of 32*UC float4 of their rows), A*UC = 16: a lane issues 16 independent
+//     16-byte loads per item; (A, UC) = (2, 8) for long rows ... (16, 1) for short ones.  Items are dealt round-robin to
+//     the warps, so the rounds are full whatever M/G is; the per-item partial dots go to shared memory and are added
+//     per atom in ascending chunk order (deterministic), then the packed argmax (Eq. 16).
+//   * one item per warp is always in flight: the first item of the next iteration is requested BEFORE the grid
+//     barrier (the dictionary never changes), so the stream does not drain at the iteration boundary.
+//   * everything after the dots (block argmax -> red.max.u64 -> ONE grid barrier -> Eq. 11 on the CTA's own float64
+//     residual with Eq. 18 as a direct sum -> stop test) is the scheme of algo 1.
+#include "mp_common.cuh"
+#include "mp_internal.h"
+
+namespace mp {
+
+constexpr int kLdgMaxWarps = 32;
+
+struct LdgParams {
+    const float* psi_t;
+    const float* y;
+    float* x;
+    float* r;
+    int* n_iter;
+    int* idx_trace;
+    float* c_trace;
+    double* x64;
+    unsigned long long* ctrl;   // [0] barrier counter, [1..3] rotating key slots
+    int64_t ld;
+    int N, M, Npad, Nr;
+    float eps;
+    int max_iter;
+};
+
+__device__ __forceinline__ float4 ldg_cg4(const float4* p)
+{
+    float4 v;
+    asm volatile("ld.global.cg.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
+    return v;
+}
+
+// A atoms x UC float4 per lane: 16 independent 16-byte loads per lane per item.  (2, 8) for long rows, (16, 1) for short ones.
+template <int A, int UC>
+__global__ void __launch_bounds__(512, 1)
+mp_persistent_ldg_kernel(const LdgParams p)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int THREADS = blockDim.x, W = THREADS >> 5;
+    const int G = gridDim.x;
+
+    double* r64 = reinterpret_cast<double*>(smem_raw);                         // Nr doubles (master residual)
+    float* r32 = reinterpret_cast<float*>(r64 + p.Nr);                         // Nr floats (fp32 rounding, feeds the dots)
+    unsigned long long* wkey = reinterpret_cast<unsigned long long*>(r32 + p.Nr);
+    double* red = reinterpret_cast<double*>(wkey + kLdgMaxWarps);
+    unsigned long long* skey = reinterpret_cast<unsigned long long*>(red + kLdgMaxWarps);
+    float* part = reinterpret_cast<float*>(skey + 2);                          // [atom of this CTA][chunk] partial dots
+
+    const int a0 = (int)(((int64_t)blockIdx.x * p.M) / G);
+    const int a1 = (int)(((int64_t)(blockIdx.x + 1) * p.M) / G);
+    const int n_atoms = a1 - a0;
+    const int n_groups = (n_atoms + A - 1) / A;
+    const int n4 = p.Npad >> 2;
+    const int n_chunks = (n4 + 32 * UC - 1) / (32 * UC);
+    const int n_items = n_groups * n_chunks;
+    const bool ragged = p.Npad != p.N;
+
+    // ---- Eq. 8: r <- y (float64 master + fp32 copy), ||y||^2 -------------------------------------------------------
+    double ss = 0.0;
+    for (int n = tid; n < p.Nr; n += THREADS) {
+        const float v = n < p.N ? p.y[n] : 0.f;
+        r64[n] = (double)v;
+        r32[n] = v;
+        ss += (double)v * (double)v;
+    }
+    ss = warp_sum(ss);
+    if (lane == 0) red[warp] = ss;
+    __syncthreads();
+    double rr = 0.0;
+    for (int w = 0; w < W; w++) rr += red[w];
+    const double yy = rr;
+    const double thresh = (double)p.eps * sqrt(yy);
+    __syncthreads();
+
+    const float4* r4 = reinterpret_cast<const float4*>(r32);
+    float4 v[A][UC];
+    auto load_item = [&](int item) {
+        const int g = item / n_chunks, ch = item - g * n_chunks;
+        const int jb = ch * 32 * UC + lane;
+#pragma unroll
+        for (int a = 0; a < A; a++) {
+            const int rel = g * A + a < n_atoms ? g * A + a : n_atoms - 1;      // a short last group re-reads its last atom
+            const float4* row = reinterpret_cast<const float4*>(p.psi_t + (int64_t)(a0 + rel) * p.ld);
+#pragma unroll
+            for (int u = 0; u < UC; u++) {
+                const int j = jb + 32 * u;
+                v[a][u] = j < n4 ? ldg_cg4(row + j) : make_float4(0.f, 0.f, 0.f, 0.f);
+            }
+        }
+    };
+    int it = warp;
+    bool have = it < n_items;
+    if (have) load_item(it);
+    int t = 0;
+    // ---- the loop: while ||r|| > eps ||y|| and t < T -----------------------------------------------------------
+    while ((sqrt(rr) > thresh) && (t < p.max_iter)) {
+        // ---------- Eq. 9: items = (group of A atoms, chunk of 32*UC float4), dealt round-robin to the warps --------------
+        // One item is always in flight per warp: `v` was loaded before the previous iteration's barrier (or in the
+        // prologue), so the stream does not drain while the CTAs meet and update the residual.
+        while (have) {
+            const int g = it / n_chunks, ch = it - g * n_chunks;
+            const int atom0 = g * A;                                           // relative to a0
+            const int jb = ch * 32 * UC + lane;
+            float acc[A];
+#pragma unroll
+            for (int a = 0; a < A; a++) acc[a] = 0.f;
+#pragma unroll
+            for (int u = 0; u < UC; u++) {
+                const int j = jb + 32 * u;
+                float4 rv = j < n4 ? r4[j] : make_float4(0.f, 0.f, 0.f, 0.f);
+                if (ragged && j == n4 - 1) {                                   // N % 4 != 0: up to 3 caller-owned pad floats per row
+                    const int n = j << 2;
+#pragma unroll
+                    for (int a = 0; a < A; a++) {
+                        if (n + 1 >= p.N) v[a][u].y = 0.f;
+                        if (n + 2 >= p.N) v[a][u].z = 0.f;
+                        v[a][u].w = 0.f;
+                    }
+                }
+#pragma unroll
+                for (int a = 0; a < A; a++) {
+                    acc[a] = fmaf(v[a][u].x, rv.x, acc[a]); acc[a] = fmaf(v[a][u].y, rv.y, acc[a]);
+                    acc[a] = fmaf(v[a][u].z, rv.z, acc[a]); acc[a] = fmaf(v[a][u].w, rv.w, acc[a]);
+                }
+            }
+            it += W;
+            have = it < n_items;
+            if (have) load_item(it);
+#pragma unroll
+            for (int a = 0; a < A; a++) {
+                const float c = warp_sum(acc[a]);
+                if (lane == a && atom0 + a < n_atoms) part[(atom0 + a) * n_chunks + ch] = c;
+            }
+        }
+        it = warp;                                                             // the dictionary never changes: the first item of
+        have = it < n_items;                                                   // the next iteration is requested ahead of the barrier
+        if (have) load_item(it);
+        __syncthreads();
+        // ---------- Eq. 9 finished per atom (chunks added in ascending order), Eq. 16 packed argmax ----------------------
+        unsigned long long best = 0ull;
+        for (int a = tid; a < n_atoms; a += THREADS) {
+            float c = part[a * n_chunks];
+            for (int ch = 1; ch < n_chunks; ch++) c += part[a * n_chunks + ch];
+            const unsigned long long k = pack_key(c, a0 + a);
+            best = k > best ? k : best;
+        }
+        best = warp_max(best);
+
+        // ---------- block argmax -> grid argmax, ONE grid barrier -------------------------------------------------
+        if (lane == 0) wkey[warp] = best;
+        __syncthreads();
+        if (warp == 0) {
+            unsigned long long k = lane < W ? wkey[lane] : 0ull;
+            k = warp_max(k);
+            if (lane == 0) {
+                unsigned long long* slot_key = p.ctrl + 1 + (t % 3);
+                if (k) red_max_u64(slot_key, k);
+                red_add_release_u64(p.ctrl, 1ull);
+                const unsigned long long target = (unsigned long long)(t + 1) * (unsigned long long)G;
+                while (ld_acquire_u64(p.ctrl) < target) {}
+                *skey = ld_relaxed_u64(slot_key);
+            }
+        }
+        __syncthreads();
+        const unsigned long long key = *skey;
+        const int i = key_index(key);
+        const float c = key_value(key);
+        const double cd = (double)c;
+
+        // ---------- Eq. 11 on this CTA's float64 r, Eq. 18 direct sum ------------------------------------------------
+        {
+            const float4* psi4 = reinterpret_cast<const float4*>(p.psi_t + (int64_t)i * p.ld);
+            double s2 = 0.0;
+            for (int j = tid; j < n4; j += THREADS) {
+                const float4 q = __ldg(psi4 + j);
+                const int n = j << 2;
+                double v0 = r64[n] - cd * (double)q.x;
+                double v1 = r64[n + 1] - cd * (double)q.y;
+                double v2 = r64[n + 2] - cd * (double)q.z;
+                double v3 = r64[n + 3] - cd * (double)q.w;
+                if (n + 3 >= p.N) {                                             // keep the pad of r at zero
+                    if (n + 1 >= p.N) v1 = 0.0;
+                    if (n + 2 >= p.N) v2 = 0.0;
+                    v3 = 0.0;
+                }
+                r64[n] = v0; r64[n + 1] = v1; r64[n + 2] = v2; r64[n + 3] = v3;
+                *reinterpret_cast<float4*>(r32 + n) = make_float4((float)v0, (float)v1, (float)v2, (float)v3);
+                s2 += v0 * v0; s2 += v1 * v1; s2 += v2 * v2; s2 += v3 * v3;
+            }
+            s2 = warp_sum(s2);
+            if (lane == 0) red[warp] = s2;
+        }
+        // ---------- Eq. 10, Eq. 12, traces: CTA 0 only ---------------------------------------------------------------
+        if (blockIdx.x == 0 && tid == 0) {
+            red_add_f64(p.x64 + i, cd);
+            if (p.idx_trace) p.idx_trace[t] = i;
+            if (p.c_trace) p.c_trace[t] = c;
+            st_relaxed_u64(p.ctrl + 1 + ((t + 2) % 3), 0ull);                   // slot of iteration t-1: everyone has read it
+        }
+        __syncthreads();
+        rr = 0.0;
+        for (int w = 0; w < W; w++) rr += red[w];
+        t += 1;
+    }
+
+    // ---- P:86 return x~ (and r, t): CTA 0 -------------------------------------------------------------------------------
+    if (blockIdx.x == 0) {
+        if (tid == 0) __threadfence();
+        __syncthreads();
+        for (int m = tid; m < p.M; m += THREADS) p.x[m] = (float)__ldcg(p.x64 + m);
+        for (int n = tid; n < p.N; n += THREADS) p.r[n] = r32[n];
+        if (tid == 0) *p.n_iter = t;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+struct LdgPlan {
+    int A, UC, W, grid;
+    size_t smem;
+};
+
+static bool ldg_plan(int N, int M, const DeviceInfo& di, LdgPlan* plan)
+{
+    const int n4 = round_up(N, 4) / 4;
+    int A = 2, UC = 8;
+    if (n4 <= 32) { A = 16; UC = 1; }
+    else if (n4 <= 64) { A = 8; UC = 2; }
+    else if (n4 <= 128) { A = 4; UC = 4; }
+    const int G = di.sm_count > 0 ? di.sm_count : 1;
+    const int atoms_max = (M + G - 1) / G;
+    const int n_chunks = (n4 + 32 * UC - 1) / (32 * UC);
+    const int items = ((atoms_max + A - 1) / A) * n_chunks;
+    const size_t Nr = (size_t)round_up(N, 128);
+    const size_t smem = Nr * 12 + 8 * (2 * kLdgMaxWarps + 4) + 4 * (size_t)atoms_max * n_chunks + 64;
+    if (smem > (size_t)di.smem_optin) return false;
+    // warps: the fullest rounds (see mp_persistent.cu make_plan); 8..16 warps, ties to more warps
+    int W = 16;
+    if (options().warps >= 1 && options().warps <= 16) W = (int)options().warps;
+    else {
+        double best = -1.0;
+        for (int w = 8; w <= 16; w++) {
+            const double fill = (double)items / ((double)((items + w - 1) / w) * w);
+            if (fill >= best) { best = fill; W = w; }
+        }
+    }
+    plan->A = A; plan->UC = UC; plan->W = W; plan->smem = smem;
+    plan->grid = options().grid > 0 && options().grid < di.sm_count ? (int)options().grid : di.sm_count;
+    return true;
+}
+
+bool persistent_ldg_supported(int N, int M)
+{
+    DeviceInfo di;
+    if (device_info(&di) != MP_OK || !di.coop) return false;
+    LdgPlan plan;
+    return ldg_plan(N, M, di, &plan);
+}
+
+template <int A, int UC>
+static mp_status launch_ldg(const LdgParams& p, const LdgPlan& plan, int device, cudaStream_t stream)
+{
+    static thread_local int attr_dev = -1;
+    if (attr_dev != device) {
+        MP_CUDA(cudaFuncSetAttribute(mp_persistent_ldg_kernel<A, UC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(227 * 1024)));
+        attr_dev = device;
+    }
+    int occ = 0;
+    MP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, mp_persistent_ldg_kernel<A, UC>, plan.W * 32, plan.smem));
+    if (occ < 1) return fail(MP_ERR_UNSUPPORTED, "register-streaming persistent kernel does not fit one CTA per SM");
+    void* args[] = {(void*)&p};
+    MP_CUDA(cudaLaunchCooperativeKernel((const void*)mp_persistent_ldg_kernel<A, UC>, dim3(plan.grid), dim3(plan.W * 32), args,
+                                        plan.smem, stream));
+    count_launch();
+    return MP_OK;
+}
+
+mp_status launch_recover_persistent_ldg(const RecoverArgs& a, const Workspace& ws, cudaStream_t stream)
+{
+    DeviceInfo di;
+    mp_status st = device_info(&di);
+    if (st != MP_OK) return st;
+    if (!di.coop) return fail(MP_ERR_UNSUPPORTED, "device does not support cooperative launch");
+    LdgPlan plan;
+    if (!ldg_plan(a.N, a.M, di, &plan)) return fail(MP_ERR_UNSUPPORTED, "N=%d, M=%d do not fit the register-streaming kernel's shared memory", a.N, a.M);
+
+    MP_CUDA(cudaMemsetAsync(ws.ctrl, 0, 256 + sizeof(double) * (size_t)a.M, stream));
+    LdgParams p;
+    p.psi_t = a.psi_t; p.y = a.y; p.x = a.x; p.r = a.r; p.n_iter = a.n_iter;
+    p.idx_trace = a.idx_trace; p.c_trace = a.c_trace;
+    p.x64 = ws.x64; p.ctrl = ws.ctrl; p.ld = a.ld;
+    p.N = a.N; p.M = a.M; p.Npad = round_up(a.N, 4); p.Nr = round_up(a.N, 128);
+    p.eps = a.eps; p.max_iter = a.max_iter;
+    if (plan.A == 16) return launch_ldg<16, 1>(p, plan, di.device, stream);
+    if (plan.A == 8) return launch_ldg<8, 2>(p, plan, di.device, stream);
+    if (plan.A == 4) return launch_ldg<4, 4>(p, plan, di.device, stream);
+    return launch_ldg<2, 8>(p, plan, di.device, stream);
+}
+
+}  // namespace mp

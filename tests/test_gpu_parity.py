@@ -41,7 +41,7 @@ def run_single(mp, psi32, y32, eps, max_iter, algo=0, ld=None):
     return (res.x.cpu().numpy(), res.r.cpu().numpy(), t, res.idx_trace.cpu().numpy()[:t], res.c_trace.cpu().numpy()[:t])
 
 
-ALGOS = [1, 2]
+ALGOS = [1, 2, 3]      # 1 = TMA-staged persistent kernel, 2 = stream loop, 3 = register-streaming persistent kernel
 
 
 # ------------------------------------------------------------------------------------------ normalisation (a0)
