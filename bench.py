@@ -296,7 +296,7 @@ def main():
     achieved = alg_bytes / (solve_ms * 1e-3) / 1e9
     per_it = ncu_traffic_per_iteration() if args.config == "cfg3" else None
     if not (B > 1 and mp.mp_get_int("info_tc_clusters")):
-      roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+      roofline = {"bound": "hbm", "regime": "hbm-streaming" if 4.0 * N * M > 126e6 else "l2-resident (frac is against the HBM peak: > 1 means served from L2)", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": per_it * its_max if per_it else None, "peak_source": peak_src,
                 "kernel": mp_kernel_name(mp), "algorithmic_bytes_per_launch": alg_bytes, "kernel_ms": solve_ms,
                 "us_per_iteration": 1e3 * solve_ms / max(its_max, 1)}
@@ -357,7 +357,8 @@ def mp_kernel_name(mp):
         if mp.mp_get_int("info_tc_clusters"):
             return ("mp_batched_tc_kernel (%d clusters x 4 CTAs, %d atoms/tile, %d stages)"
                     % (mp.mp_get_int("info_tc_clusters"), mp.mp_get_int("info_tc_at"), mp.mp_get_int("info_tc_stages")))
-        return {0: "auto", 1: "mp_persistent_kernel", 2: "stream loop"}[mp.mp_get_int("algo")]
+        return {1: "mp_persistent_kernel (TMA-staged)", 2: "stream loop",
+                3: "mp_persistent_ldg_kernel (register-streaming)"}[mp.mp_get_int("info_algo")]
     except Exception:
         return "?"
 

@@ -132,6 +132,7 @@ static int64_t* option_slot(const char* name)
     if (!strcmp(name, "chunk")) return &o.chunk;
     if (!strcmp(name, "batched_algo")) return &o.batched_algo;
     if (!strcmp(name, "batched_coop")) return &o.batched_coop;
+    if (!strcmp(name, "info_algo")) return &o.info_algo;
     if (!strcmp(name, "info_tc_clusters")) return &o.info_tc_clusters;
     if (!strcmp(name, "info_tc_at")) return &o.info_tc_at;
     if (!strcmp(name, "info_tc_stages")) return &o.info_tc_stages;
@@ -183,11 +184,11 @@ mp_status mp_recover(const float* psi_t, int N, int M, int64_t ld,
     RecoverArgs a{psi_t, N, M, ld, y, eps, max_iter, x, r, n_iter, idx_trace, c_trace};
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     const int64_t algo = options().algo;
-    if (algo == 2) return launch_recover_streamloop(a, ws, s);
-    if (algo == 1) return launch_recover_persistent(a, ws, s);
-    if (algo == 3) return launch_recover_persistent_ldg(a, ws, s);
-    if (persistent_ldg_supported(N, M)) return launch_recover_persistent_ldg(a, ws, s);
-    if (persistent_supported(N, M)) return launch_recover_persistent(a, ws, s);
+    int64_t use = algo;
+    if (use < 1 || use > 3) use = persistent_ldg_supported(N, M) ? 3 : persistent_supported(N, M) ? 1 : 2;
+    options().info_algo = use;
+    if (use == 3) return launch_recover_persistent_ldg(a, ws, s);
+    if (use == 1) return launch_recover_persistent(a, ws, s);
     return launch_recover_streamloop(a, ws, s);
 }
 
