@@ -89,7 +89,7 @@ __device__ __forceinline__ void tc_grid_barrier(unsigned long long* counter, uns
 }
 
 // Split-TF32 operands.  kind::tf32 reads fp32 words and uses their top 19 bits (sign, exponent, 10 mantissa bits).
-//   dictionary: hi = the raw word as the tensor core sees it (low 13 bits ignored), lo = rn_tf32(psi - trunc(psi));
+//   dictionary: hi = the raw word as the tensor core sees it (low 13 bits ignored), lo = rn_tf32(psi - trunc(psi)) (Dekker split, tf32_rn_split);
 //   residual:   hi = rn_tf32(r), lo = rn_tf32(r - hi).
 // The low parts are rounded to nearest HERE, so the hardware conversion of them is exact and the remaining
 // representation error (<= 2^-22 |psi|, <= 2^-23 |r|) has no systematic sign: it averages out over the dot product
@@ -100,6 +100,15 @@ __device__ __forceinline__ float tf32_rn(float v)
     uint32_t o;
     asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(o) : "f"(v));
     return __uint_as_float(o);
+}
+
+// round to 11 significant bits (tf32-exact) with Dekker's splitting, 3 flops instead of the multi-instruction
+// cvt.rna.tf32.f32: c = 8193 v; hi = c - (c - v).  Exact for the dictionary low parts (|v| < 2^-10, no overflow; a
+// subnormal v comes back unchanged or rounded, either way tf32-exact enough: the hardware ignores what is left).
+__device__ __forceinline__ float tf32_rn_split(float v)
+{
+    const float c = __fmul_rn(v, 8193.0f);
+    return __fsub_rn(c, __fsub_rn(c, v));
 }
 
 // block-wide float64 sum in a fixed order (all threads of the CTA call; result uniform)
@@ -304,8 +313,8 @@ mp_batched_tc_kernel(const __grid_constant__ CUtensorMap tm_psi, const __grid_co
                     mbar_wait(&tail->lo_empty[h], (uint32_t)(((g_wrk >> 1) & 1) ^ 1));
                     for (int i = wtid; i < p.AT * 8; i += kTcWorkers) {
                         const float4 v = raw[i];
-                        lo[i] = make_float4(tf32_rn(v.x - tf32_trunc(v.x)), tf32_rn(v.y - tf32_trunc(v.y)),
-                                            tf32_rn(v.z - tf32_trunc(v.z)), tf32_rn(v.w - tf32_trunc(v.w)));
+                        lo[i] = make_float4(tf32_rn_split(v.x - tf32_trunc(v.x)), tf32_rn_split(v.y - tf32_trunc(v.y)),
+                                            tf32_rn_split(v.z - tf32_trunc(v.z)), tf32_rn_split(v.w - tf32_trunc(v.w)));
                     }
                     fence_proxy_async_smem();
                     __syncwarp();
