@@ -119,6 +119,17 @@ MP_API mp_status mp_correlate_batched(const float* psi_t, int N, int M, int64_t 
                                const float* Y, int64_t ldy, int B, float* C,
                                void* workspace, size_t workspace_bytes, void* stream);
 
+/* ---- the steps either side of the path: encode and score on the device ------------------
+ * mp_encode_sparse, Eq. 2: y = Psi x for a K-sparse x given as K (index, value) pairs, the way the paper
+ * builds x (A2 P:328-332):   y[n] = sum_{k<K} val[k] * psi_t[idx[k]*ld + n],   ascending k, float64 accumulation,
+ * one rounding to fp32.  Reads 4NK bytes instead of the 4NM of a dense product.  idx (K ints, device) is 0-based;
+ * repeated indices accumulate; an index outside [0, M) contributes nothing.  K = 0 gives y = 0.
+ * mp_reconstruction_error, Eq. 14: err_pct[0] = 100 * ||x_hat - x||_2^2 / ||x||_2^2 (one double, device,
+ * 8-byte aligned), float64 sums in a fixed order.  x = 0 gives NaN or +inf as the formula does. */
+MP_API mp_status mp_encode_sparse(const float* psi_t, int N, int M, int64_t ld, const int* idx, const float* val, int K,
+                           float* y, void* stream);
+MP_API mp_status mp_reconstruction_error(const float* x_hat, const float* x, int M, double* err_pct, void* stream);
+
 /* Description of the last error on this thread ("" if none).  Static storage, never NULL. */
 MP_API const char* mp_last_error(void);
 

@@ -74,6 +74,20 @@ int oracle_mp_batched_f32(const float* psi_t, int N, int M, int64_t ld, const do
     return 0;
 }
 
+/* Eq. 2: y = Psi x, x K-sparse as (idx, val) pairs; one serial ascending-k sum per component. */
+int oracle_encode_sparse_f32(const float* psi_t, int N, int M, int64_t ld, const int* idx, const double* val, int K, double* y)
+{
+    if (!psi_t || !y || N < 1 || M < 1 || K < 0 || ld < N || (K > 0 && (!idx || !val))) return 1;
+    for (int k = 0; k < K; k++)
+        if (idx[k] < 0 || idx[k] >= M) return 1;
+    for (int n = 0; n < N; n++) {
+        double s = 0.0;
+        for (int k = 0; k < K; k++) s += val[k] * (double)psi_t[(int64_t)idx[k] * ld + n];
+        y[n] = s;
+    }
+    return 0;
+}
+
 /* Eq. 14: E = ||x~ - x||^2 ||x||^-2 x 100%. */
 double oracle_reconstruction_error_pct(const double* x_hat, const double* x, int M)
 {

@@ -87,6 +87,11 @@ int oracle_mp_replay_f32(const float* psi_t, int N, int M, int64_t ld, const dou
 int oracle_mp_batched_f32(const float* psi_t, int N, int M, int64_t ld, const double* Y, int64_t ldy, int B,
                           double eps, int T, double* X, double* R, int* n_iter, int nthreads);
 
+/* Eq. 2: y = Psi x for a K-sparse x given as (index, value) pairs (the paper builds x that way, A2 P:328-332):
+ *   y[n] = sum_{k=0}^{K-1} val[k] * Psi[n][idx[k]],  ascending k, float64.  Repeated indices accumulate (the paper's
+ * rand()%M support can repeat).  Returns 0, or 1 on invalid arguments (an index outside [0, M)). */
+int oracle_encode_sparse_f32(const float* psi_t, int N, int M, int64_t ld, const int* idx, const double* val, int K, double* y);
+
 /* Eq. 14: E = ||x_hat - x||_2^2 / ||x||_2^2 * 100 (percent). */
 double oracle_reconstruction_error_pct(const double* x_hat, const double* x, int M);
 

@@ -15,7 +15,7 @@ import numpy as np
 from . import build as _build
 
 __all__ = ["normalize_columns", "correlate", "argmax_abs", "nrm2", "mp", "mp_replay",
-           "mp_batched", "reconstruction_error_pct", "MPResult", "ReplayResult", "default_threads"]
+           "mp_batched", "encode_sparse", "reconstruction_error_pct", "MPResult", "ReplayResult", "default_threads"]
 
 _lib = C.CDLL(_build.build())
 
@@ -45,6 +45,8 @@ for _s in ("f64", "f32"):
 _lib.oracle_mp_batched_f32.restype = C.c_int
 _lib.oracle_mp_batched_f32.argtypes = [_vp, C.c_int, C.c_int, C.c_int64, _vp, C.c_int64, C.c_int,
                                        C.c_double, C.c_int, _vp, _vp, _vp, C.c_int]
+_lib.oracle_encode_sparse_f32.restype = C.c_int
+_lib.oracle_encode_sparse_f32.argtypes = [_vp, C.c_int, C.c_int, C.c_int64, _vp, _vp, C.c_int, _vp]
 _lib.oracle_reconstruction_error_pct.restype = C.c_double
 _lib.oracle_reconstruction_error_pct.argtypes = [_vp, _vp, C.c_int]
 
@@ -186,6 +188,20 @@ def mp_batched(psi_t, Y, eps: float, max_iter: int, nthreads: int = 1):
     if rc:
         raise ValueError("oracle_mp_batched: invalid arguments")
     return X, R, n_iter
+
+
+def encode_sparse(psi_t, idx, val) -> np.ndarray:
+    """Eq. 2: y[n] = sum_k val[k] * Psi[n][idx[k]] (ascending k, float64) from the float32 dictionary."""
+    a, s, N, M, ld = _psi(psi_t)
+    if s != "f32":
+        raise TypeError("encode_sparse takes the float32 dictionary")
+    idx = np.ascontiguousarray(idx, dtype=np.int32)
+    val = _f64(val)
+    assert idx.size == val.size
+    y = np.empty(N, dtype=np.float64)
+    if _lib.oracle_encode_sparse_f32(_ptr(a), N, M, ld, _ptr(idx), _ptr(val), int(idx.size), _ptr(y)):
+        raise ValueError("oracle_encode_sparse: invalid arguments")
+    return y
 
 
 def reconstruction_error_pct(x_hat, x) -> float:

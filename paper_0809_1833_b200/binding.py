@@ -54,6 +54,10 @@ lib.mp_correlate_batched_workspace_bytes.restype = _sz
 lib.mp_correlate_batched_workspace_bytes.argtypes = [_i, _i, _i]
 lib.mp_correlate_batched.restype = _i
 lib.mp_correlate_batched.argtypes = [_vp, _i, _i, _i64, _vp, _i64, _i, _vp, _vp, _sz, _vp]
+lib.mp_encode_sparse.restype = _i
+lib.mp_encode_sparse.argtypes = [_vp, _i, _i, _i64, _vp, _vp, _i, _vp, _vp]
+lib.mp_reconstruction_error.restype = _i
+lib.mp_reconstruction_error.argtypes = [_vp, _vp, _i, _vp, _vp]
 lib.mp_last_error.restype = C.c_char_p
 lib.mp_last_error.argtypes = []
 lib.mp_set_int.restype = _i
@@ -215,6 +219,31 @@ def mp_correlate_batched(psi_t: torch.Tensor, Y: torch.Tensor, *, C_out=None, st
                                         base + off, ws.numel() - off, _stream_ptr(stream)))
     C_out._mp_workspace = ws          # keep the workspace alive until the stream has run the kernel
     return C_out
+
+
+def mp_encode_sparse(psi_t: torch.Tensor, idx: torch.Tensor, val: torch.Tensor, *, y=None, stream=None) -> torch.Tensor:
+    """Eq. 2: y = Psi x for a K-sparse x given as (idx int32[K], val float32[K]) device tensors."""
+    p, N, M, ld = _dict_args(psi_t)
+    K = idx.numel()
+    if val.numel() != K:
+        raise ValueError("idx and val must have the same length")
+    y = torch.empty(N, dtype=torch.float32, device=psi_t.device) if y is None else y
+    with torch.cuda.device(psi_t.device):
+        _check(lib.mp_encode_sparse(p, N, M, ld, _dev(idx, torch.int32, "idx") if K else None,
+                                    _dev(val, torch.float32, "val") if K else None, K, _dev(y, torch.float32, "y"),
+                                    _stream_ptr(stream)))
+    return y
+
+
+def mp_reconstruction_error(x_hat: torch.Tensor, x: torch.Tensor, *, out=None, stream=None) -> torch.Tensor:
+    """Eq. 14: 100 * ||x_hat - x||^2 / ||x||^2 as a float64[1] device tensor."""
+    if x_hat.numel() != x.numel():
+        raise ValueError("x_hat and x must have the same length")
+    out = torch.empty(1, dtype=torch.float64, device=x.device) if out is None else out
+    with torch.cuda.device(x.device):
+        _check(lib.mp_reconstruction_error(_dev(x_hat, torch.float32, "x_hat"), _dev(x, torch.float32, "x"), x.numel(),
+                                           _dev(out, torch.float64, "err_pct"), _stream_ptr(stream)))
+    return out
 
 
 def _host(t: torch.Tensor, dtype, what: str):

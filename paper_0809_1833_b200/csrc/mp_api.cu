@@ -163,6 +163,24 @@ mp_status mp_normalize_columns(float* psi_t, int N, int M, int64_t ld, float* no
     return launch_normalize(psi_t, N, M, ld, norms_out, static_cast<cudaStream_t>(stream));
 }
 
+mp_status mp_encode_sparse(const float* psi_t, int N, int M, int64_t ld, const int* idx, const float* val, int K,
+                           float* y, void* stream)
+{
+    mp_status st = check_dictionary(psi_t, N, M, ld);
+    if (st != MP_OK) return st;
+    if (K < 0) return fail(MP_ERR_INVALID_ARG, "need K >= 0 (got %d)", K);
+    if (!y || (K > 0 && (!idx || !val))) return fail(MP_ERR_INVALID_ARG, "y (and idx, val when K > 0) must be non-null");
+    return launch_encode_sparse(psi_t, N, M, ld, idx, val, K, y, static_cast<cudaStream_t>(stream));
+}
+
+mp_status mp_reconstruction_error(const float* x_hat, const float* x, int M, double* err_pct, void* stream)
+{
+    if (!x_hat || !x || !err_pct) return fail(MP_ERR_INVALID_ARG, "x_hat, x and err_pct must be non-null");
+    if (M < 1) return fail(MP_ERR_INVALID_ARG, "need M >= 1 (got %d)", M);
+    if (reinterpret_cast<uintptr_t>(err_pct) & 7u) return fail(MP_ERR_INVALID_ARG, "err_pct must be 8-byte aligned");
+    return launch_reconstruction_error(x_hat, x, M, err_pct, static_cast<cudaStream_t>(stream));
+}
+
 mp_status mp_recover(const float* psi_t, int N, int M, int64_t ld,
                      const float* y, float eps, int max_iter,
                      float* x, float* r, int* n_iter,

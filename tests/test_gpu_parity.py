@@ -326,6 +326,50 @@ def test_cfg5_full_size_batched_grading(mp):
     print(f"cfg5 worst step-value error {worst:.3e} ||r|| (tolerance {c_tol:.3e})")
 
 
+# ------------------------------------------------------------------------------------------ encode + score on device (NEXT 1)
+@pytest.mark.parametrize("N,M,K", [(256, 1024, 16), (250, 333, 8), (4096, 16384, 256), (37, 1000, 700), (2048, 8192, 0)])
+def test_encode_sparse_is_bit_exact(mp, N, M, K):
+    """Eq. 2: the device encode equals the oracle's ascending-k float64 sum rounded to fp32 once, bit for bit (the
+    products double(float)*double(float) are exact, the adds run in the same order)."""
+    cfg = problems.custom_config(N, M, max(K, 1))
+    psi32 = problems.normalise_on_host(synth.make_dictionary(cfg, seed=4))
+    rng = np.random.default_rng(9)
+    idx = rng.integers(0, M, K).astype(np.int32)                             # with replacement: repeats accumulate
+    val = rng.standard_normal(K).astype(np.float32)
+    ld = (N + 3) // 4 * 4
+    buf = torch.full((M, ld), 3.0, dtype=torch.float32, device="cuda"); buf[:, :N] = dev(psi32)
+    y = mp.mp_encode_sparse(buf[:, :N], dev(idx), dev(val))
+    torch.cuda.synchronize()
+    ref = oracle.encode_sparse(psi32, idx, val.astype(np.float64)).astype(np.float32)
+    assert np.array_equal(y.cpu().numpy(), ref)
+    if K:                                                                    # an out-of-range index contributes nothing
+        bad = idx.copy(); bad[0] = M + 5
+        y2 = mp.mp_encode_sparse(buf[:, :N], dev(bad), dev(val)).cpu().numpy()
+        ref2 = oracle.encode_sparse(psi32, idx[1:], val[1:].astype(np.float64)).astype(np.float32)
+        assert np.array_equal(y2, ref2)
+
+
+def test_encode_recover_score_pipeline_on_device(mp):
+    """encode -> mp_recover -> score without host data (CFG1): the recovered x~ scores Eq. 14 like the oracle's
+    formula on the same vectors, and the error is at the "recovers exactly" level."""
+    pb = problems.make_problem(synth.config("cfg1"), 2)
+    c = pb.cfg
+    psi_d = dev(pb.psi32)
+    order = np.sort(pb.S[0])
+    y_d = mp.mp_encode_sparse(psi_d, dev(order.astype(np.int32)), dev(pb.X[0][order].astype(np.float32)))
+    x32 = pb.X[0][order].astype(np.float32)                                  # the device encode takes fp32 coefficients
+    assert np.array_equal(y_d.cpu().numpy(), oracle.encode_sparse(pb.psi32, order, x32.astype(np.float64)).astype(np.float32))
+    res = mp.mp_recover(psi_d, y_d, c.eps, c.max_iter)
+    x_true_d = dev(pb.X[0].astype(np.float32))
+    e = mp.mp_reconstruction_error(res.x, x_true_d)
+    torch.cuda.synchronize()
+    ref = oracle.reconstruction_error_pct(res.x.cpu().numpy().astype(np.float64), pb.X[0].astype(np.float32).astype(np.float64))
+    assert abs(e.item() - ref) <= 1e-12 * ref and e.item() < 1e-6
+    # a hand-computed case: (0.1^2 + 0.1^2) / 1 * 100 = 2 %
+    e2 = mp.mp_reconstruction_error(dev(np.array([0.9, 0.1, 0.0], np.float32)), dev(np.array([1.0, 0.0, 0.0], np.float32)))
+    assert abs(e2.item() - 2.0) < 1e-5
+
+
 # ------------------------------------------------------------------------------------------ host-buffer entry points (e2e path)
 def test_host_entry_point_matches_device_entry_point(mp):
     pb = problems.make_problem(synth.config("cfg1"), 3)

@@ -409,3 +409,37 @@ def test_paper_sweep_parameters_finish_within_T_and_recover_x(M, seed):
     assert oracle.reconstruction_error_pct(res.x, x) < 1e-3
     full = oracle.mp(psi_t, y, 0.0, T)                      # exactly T = N steps
     assert oracle.reconstruction_error_pct(full.x, x) < 1e-5   # "recovers exactly"
+
+
+# ----------------------------------------------------------------------------- Eq. 2 (encode), the step before the path
+def test_encode_sparse_pins():
+    """Eq. 2, y = Psi x for a K-sparse x: a unit coefficient returns the atom itself; the result equals numpy's
+    float64 dense product Psi^T-major @ x to rounding; a brute-force Python double loop on a tiny case is matched exactly;
+    repeated indices accumulate (A2 P:328-332 draws the support with replacement); power-of-two scaling is exact."""
+    rng = np.random.default_rng(3)
+    M, N, K = 40, 12, 5
+    psi = rng.standard_normal((M, N)).astype(np.float32)
+    for m in (0, 7, M - 1):
+        assert np.array_equal(oracle.encode_sparse(psi, [m], [1.0]), psi[m].astype(np.float64))
+    idx = rng.choice(M, K, replace=False); val = rng.standard_normal(K)
+    y = oracle.encode_sparse(psi, idx, val)
+    x = np.zeros(M); x[idx] = val
+    dense = psi.astype(np.float64).T @ x
+    assert np.allclose(y, dense, rtol=0, atol=1e-15 * np.abs(psi).max() * np.abs(val).sum())
+    brute = [sum(float(val[k]) * float(psi[idx[k], n]) for k in range(K)) for n in range(N)]
+    acc = []
+    for n in range(N):                                   # the same ascending-k order, one add at a time
+        s = 0.0
+        for k in range(K):
+            s += float(val[k]) * float(psi[idx[k], n])
+        acc.append(s)
+    assert list(y) == acc and np.allclose(y, brute, atol=1e-15)
+    assert np.array_equal(oracle.encode_sparse(psi, [3, 3], [0.5, 0.25]), 0.75 * psi[3].astype(np.float64))
+    assert np.array_equal(oracle.encode_sparse(psi, idx, 4.0 * val), 4.0 * y)
+    assert np.array_equal(oracle.encode_sparse(psi, [], []), np.zeros(N))
+    with pytest.raises(ValueError):
+        oracle.encode_sparse(psi, [M], [1.0])
+    # and it agrees with the input generator's encode (which bench.py and the parity tests use to make y)
+    from paper_0809_1833_b200 import synth
+    assert np.array_equal(y.astype(np.float32), synth.encode(psi, x, np.sort(idx))) or \
+        np.allclose(y.astype(np.float32), synth.encode(psi, x, np.sort(idx)), rtol=2e-7)
