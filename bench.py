@@ -193,6 +193,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--max-iter", type=int, default=None, help="override the config's iteration cap (profiling runs)")
+    ap.add_argument("--f64", action="store_true", help="double-precision path (mp_recover_f64) on the same workload shape")
     ap.add_argument("--knob", action="append", default=[], metavar="NAME=VALUE", help="mp_set_int knob (profiling runs)")
     args = ap.parse_args()
     cfg = synth.config(args.config)
@@ -209,6 +210,8 @@ def main():
     for kv in args.knob:
         name, _, val = kv.partition("=")
         mp.mp_set_int(name, int(val))
+    if args.f64:
+        return run_f64(args, cfg, torch, mp)
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
@@ -350,6 +353,65 @@ def main():
             "roofline": roofline, "cpu_baseline": cb, "e2e": e2e}))
     if dist:
         dist.destroy_process_group()
+
+
+def run_f64(args, cfg, torch, mp):
+    """The double-precision path (NEXT 3) on the same workload shape, 1 GPU: normalise + solve in float64, HBM roofline
+    with 8NM bytes per iteration.  Same JSON contract, dtype "f64"."""
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(0)
+    N, M = cfg.N, cfg.M
+    psi_d = torch.from_numpy(synth.make_dictionary(cfg, 1)).to(dev).double()
+    mp.mp_normalize_columns_f64(psi_d)
+    x, sup = synth.sparse_signal(M, cfg.K, 1, cfg.values, signal=0)
+    order = np.sort(sup)
+    y_d = (torch.from_numpy(x[order]).to(dev)[:, None] * psi_d[torch.from_numpy(order).to(dev)]).sum(0)
+    eps = float(np.float32(cfg.eps))
+    ws = torch.empty(mp.binding.lib.mp_workspace_bytes_f64(N, M) + 256, dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream()
+    for _ in range(args.warmup):
+        mp.mp_normalize_columns_f64(psi_d); res = mp.mp_recover_f64(psi_d, y_d, eps, cfg.max_iter, workspace=ws)
+    clocks = ClockSampler(0); clocks.start()
+    torch.cuda.synchronize()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2 * args.steps + 2)]
+    l0 = mp.mp_launch_count()
+    ev[0].record(stream)
+    for k in range(args.steps):
+        mp.mp_normalize_columns_f64(psi_d)
+        ev[2 + 2 * k].record(stream)
+        res = mp.mp_recover_f64(psi_d, y_d, eps, cfg.max_iter, workspace=ws)
+        ev[3 + 2 * k].record(stream)
+    ev[1].record(stream)
+    torch.cuda.synchronize()
+    clk = clocks.stop()
+    launches = mp.mp_launch_count() - l0
+    its = int(res.n_iter.item())
+    ms_total = ev[0].elapsed_time(ev[1])
+    solve_ms = float(np.mean([ev[2 + 2 * k].elapsed_time(ev[3 + 2 * k]) for k in range(args.steps)]))
+    peak, peak_src = load_peaks()
+    alg_bytes = its * (8.0 * N * M + 8.0 * N)
+    ach = alg_bytes / (solve_ms * 1e-3) / 1e9
+    cb = None
+    if not args.no_cpu_baseline:
+        import oracle
+        psi_h = psi_d.cpu().numpy(); y_h = y_d.cpu().numpy(); th = oracle.default_threads()
+        t0 = time.perf_counter(); oracle.mp(psi_h, y_h, eps, 4, th); per_it = (time.perf_counter() - t0) / 4
+        T = int(max(4, min(cfg.max_iter, 12.0 / per_it)))
+        t0 = time.perf_counter(); r = oracle.mp(psi_h, y_h, eps, T, th); dt = time.perf_counter() - t0
+        cb = {"value": r.n_iter / dt, "unit": UNIT, "cores": th, "kind": "oracle",
+              "sample": f"first {r.n_iter} MP iterations of {cfg.name} in float64 (C oracle, OpenMP over atoms, {th} threads)"}
+    print(json.dumps({
+        "metric": METRIC, "value": its * args.steps / (ms_total * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(cfg).replace("MP fp32", "MP fp64") + ", double precision (float64 dictionary, 8NM bytes per iteration)",
+                   "iterations_per_step": its, "step": "mp_normalize_columns_f64 + mp_recover_f64 (whole solve to the eps stop)",
+                   "l2": "dictionary 8NM = %.0f MiB" % (8.0 * N * M / 2**20), "parallelism": "1 GPU"},
+        "time_to_recovery_ms": solve_ms, "gpu_launches": int(launches), "clocks": clk,
+        "roofline": {"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "traffic": None,
+                     "peak_source": peak_src, "kernel": "mp_persistent_f64_kernel", "algorithmic_bytes_per_launch": alg_bytes,
+                     "kernel_ms": solve_ms, "us_per_iteration": 1e3 * solve_ms / max(its, 1)},
+        "cpu_baseline": cb, "e2e": None}))
 
 
 def mp_kernel_name(mp):

@@ -130,6 +130,19 @@ MP_API mp_status mp_encode_sparse(const float* psi_t, int N, int M, int64_t ld, 
                            float* y, void* stream);
 MP_API mp_status mp_reconstruction_error(const float* x_hat, const float* x, int M, double* err_pct, void* stream);
 
+/* ---- double-precision path (the paper reports both precisions) -------------
+ * The same loop on a float64 dictionary: psi_t[m*ld + n], ld >= N, ld % 2 == 0, 16-byte aligned; y, x, r, c_trace and
+ * eps are double.  All arithmetic is float64 (dots, residual, norms, coefficients); ties go to the lowest index.
+ * Workspace: mp_workspace_bytes_f64(N, M) bytes, 256-byte aligned.  One persistent cooperative kernel per solve;
+ * MP_ERR_UNSUPPORTED if the residual does not fit in shared memory (N > ~28 000).  HBM roofline: 8NM bytes per iteration. */
+MP_API size_t mp_workspace_bytes_f64(int N, int M);
+MP_API mp_status mp_normalize_columns_f64(double* psi_t, int N, int M, int64_t ld, double* norms_out, void* stream);
+MP_API mp_status mp_recover_f64(const double* psi_t, int N, int M, int64_t ld,
+                         const double* y, double eps, int max_iter,
+                         double* x, double* r, int* n_iter,
+                         int* idx_trace, double* c_trace,
+                         void* workspace, size_t workspace_bytes, void* stream);
+
 /* Description of the last error on this thread ("" if none).  Static storage, never NULL. */
 MP_API const char* mp_last_error(void);
 

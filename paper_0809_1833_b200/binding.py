@@ -58,6 +58,12 @@ lib.mp_encode_sparse.restype = _i
 lib.mp_encode_sparse.argtypes = [_vp, _i, _i, _i64, _vp, _vp, _i, _vp, _vp]
 lib.mp_reconstruction_error.restype = _i
 lib.mp_reconstruction_error.argtypes = [_vp, _vp, _i, _vp, _vp]
+lib.mp_workspace_bytes_f64.restype = _sz
+lib.mp_workspace_bytes_f64.argtypes = [_i, _i]
+lib.mp_normalize_columns_f64.restype = _i
+lib.mp_normalize_columns_f64.argtypes = [_vp, _i, _i, _i64, _vp, _vp]
+lib.mp_recover_f64.restype = _i
+lib.mp_recover_f64.argtypes = [_vp, _i, _i, _i64, _vp, C.c_double, _i, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]
 lib.mp_last_error.restype = C.c_char_p
 lib.mp_last_error.argtypes = []
 lib.mp_set_int.restype = _i
@@ -244,6 +250,47 @@ def mp_reconstruction_error(x_hat: torch.Tensor, x: torch.Tensor, *, out=None, s
         _check(lib.mp_reconstruction_error(_dev(x_hat, torch.float32, "x_hat"), _dev(x, torch.float32, "x"), x.numel(),
                                            _dev(out, torch.float64, "err_pct"), _stream_ptr(stream)))
     return out
+
+
+def _dict_args_f64(psi_t: torch.Tensor):
+    if not (psi_t.is_cuda and psi_t.dtype == torch.float64 and psi_t.dim() == 2 and (psi_t.shape[1] == 1 or psi_t.stride(1) == 1)):
+        raise TypeError("psi_t must be a CUDA float64 [M, N] tensor with unit stride along N (atom-major)")
+    M, N = psi_t.shape
+    ld = psi_t.stride(0) if M > 1 else max(psi_t.stride(0), N)
+    return psi_t.data_ptr(), N, M, ld
+
+
+def mp_normalize_columns_f64(psi_t: torch.Tensor, norms_out: torch.Tensor | None = None, stream=None) -> None:
+    """Eq. 4 in float64, in place on the device tensor psi_t[M, N]."""
+    p, N, M, ld = _dict_args_f64(psi_t)
+    n = _dev(norms_out, torch.float64, "norms_out") if norms_out is not None else None
+    with torch.cuda.device(psi_t.device):
+        _check(lib.mp_normalize_columns_f64(p, N, M, ld, n, _stream_ptr(stream)))
+
+
+def mp_recover_f64(psi_t: torch.Tensor, y: torch.Tensor, eps: float, max_iter: int, *, trace: bool = False,
+                   workspace=None, stream=None) -> Recovered:
+    """Eq. 8-12 in double precision (float64 dictionary, signal, coefficients and residual)."""
+    p, N, M, ld = _dict_args_f64(psi_t)
+    dev = psi_t.device
+    if y.numel() != N:
+        raise ValueError("y must have N elements")
+    x = torch.empty(M, dtype=torch.float64, device=dev)
+    r = torch.empty(N, dtype=torch.float64, device=dev)
+    n_iter = torch.empty(1, dtype=torch.int32, device=dev)
+    idx_trace = torch.empty(max(max_iter, 1), dtype=torch.int32, device=dev) if trace else None
+    c_trace = torch.empty(max(max_iter, 1), dtype=torch.float64, device=dev) if trace else None
+    need = lib.mp_workspace_bytes_f64(N, M)
+    if workspace is None:
+        workspace = torch.empty(need + 256, dtype=torch.uint8, device=dev)
+    base = workspace.data_ptr()
+    off = (-base) % 256
+    with torch.cuda.device(dev):
+        _check(lib.mp_recover_f64(p, N, M, ld, _dev(y, torch.float64, "y"), float(eps), int(max_iter),
+                                  x.data_ptr(), r.data_ptr(), n_iter.data_ptr(),
+                                  idx_trace.data_ptr() if trace else None, c_trace.data_ptr() if trace else None,
+                                  base + off, workspace.numel() - off, _stream_ptr(stream)))
+    return Recovered(x, r, n_iter, idx_trace, c_trace, workspace)
 
 
 def _host(t: torch.Tensor, dtype, what: str):
