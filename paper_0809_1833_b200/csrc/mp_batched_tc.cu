@@ -659,8 +659,9 @@ mp_status launch_recover_batched_tc(const BatchedArgs& a, const Workspace& ws, f
     at[1].val.cooperative = 1;
     cfg.attrs = at; cfg.numAttrs = options().batched_coop ? 2 : 1;
     cudaError_t e = cudaLaunchKernelEx(&cfg, mp_batched_tc_kernel, tm_psi, tm_rs, p);
-    if (e == cudaErrorNotSupported || e == cudaErrorInvalidValue || e == cudaErrorCooperativeLaunchTooLarge) {
-        // cluster + cooperative attribute refused: the grid is sized from cudaOccupancyMaxActiveClusters, so all
+    if (options().batched_coop && (e == cudaErrorNotSupported || e == cudaErrorInvalidValue)) {
+        // the cluster + cooperative attribute combination itself refused (not "too large": that stays an error, a grid
+        // that is not co-resident would deadlock): the grid is sized from cudaOccupancyMaxActiveClusters, so all
         // clusters are co-resident on an otherwise idle device without the attribute as well
         (void)cudaGetLastError();
         cfg.numAttrs = 1;
