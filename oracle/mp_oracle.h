@@ -87,6 +87,16 @@ int oracle_mp_replay_f32(const float* psi_t, int N, int M, int64_t ld, const dou
 int oracle_mp_batched_f32(const float* psi_t, int N, int M, int64_t ld, const double* Y, int64_t ldy, int B,
                           double eps, int T, double* X, double* R, int* n_iter, int nthreads);
 
+/* Orthogonal MP (textbook definition, see mp_oracle.c): MP's selection followed by a least-squares
+ * refit on the selected atoms (normal equations, Cholesky from scratch every iteration).  idx_force != NULL: the
+ * teacher-forced replay over t_force imposed atoms.  Returns 0, 1 (invalid arguments) or 2 (an atom selected twice or
+ * a singular Gram matrix ended the run). */
+int oracle_omp_f32(const float* psi_t, int N, int M, int64_t ld, const double* y, double eps, int T,
+                   const int* idx_force, int t_force,
+                   double* x, double* r, int* n_iter,
+                   int* idx_trace, double* gap_trace, double* rnorm_trace,
+                   int* argmax_ref, double* cmax_ref, double* c_at_idx, int nthreads);
+
 /* Eq. 2: y = Psi x for a K-sparse x given as (index, value) pairs (the paper builds x that way, A2 P:328-332):
  *   y[n] = sum_{k=0}^{K-1} val[k] * Psi[n][idx[k]],  ascending k, float64.  Repeated indices accumulate (the paper's
  * rand()%M support can repeat).  Returns 0, or 1 on invalid arguments (an index outside [0, M)). */

@@ -15,7 +15,7 @@ import numpy as np
 from . import build as _build
 
 __all__ = ["normalize_columns", "correlate", "argmax_abs", "nrm2", "mp", "mp_replay",
-           "mp_batched", "encode_sparse", "reconstruction_error_pct", "MPResult", "ReplayResult", "default_threads"]
+           "mp_batched", "omp", "OMPResult", "encode_sparse", "reconstruction_error_pct", "MPResult", "ReplayResult", "default_threads"]
 
 _lib = C.CDLL(_build.build())
 
@@ -45,6 +45,9 @@ for _s in ("f64", "f32"):
 _lib.oracle_mp_batched_f32.restype = C.c_int
 _lib.oracle_mp_batched_f32.argtypes = [_vp, C.c_int, C.c_int, C.c_int64, _vp, C.c_int64, C.c_int,
                                        C.c_double, C.c_int, _vp, _vp, _vp, C.c_int]
+_lib.oracle_omp_f32.restype = C.c_int
+_lib.oracle_omp_f32.argtypes = [_vp, C.c_int, C.c_int, C.c_int64, _vp, C.c_double, C.c_int, _vp, C.c_int,
+                                _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, C.c_int]
 _lib.oracle_encode_sparse_f32.restype = C.c_int
 _lib.oracle_encode_sparse_f32.argtypes = [_vp, C.c_int, C.c_int, C.c_int64, _vp, _vp, C.c_int, _vp]
 _lib.oracle_reconstruction_error_pct.restype = C.c_double
@@ -188,6 +191,41 @@ def mp_batched(psi_t, Y, eps: float, max_iter: int, nthreads: int = 1):
     if rc:
         raise ValueError("oracle_mp_batched: invalid arguments")
     return X, R, n_iter
+
+
+@dataclasses.dataclass
+class OMPResult:
+    x: np.ndarray            # [M] float64: least-squares coefficients on the selected atoms, 0 elsewhere
+    r: np.ndarray            # [N] float64: y - Psi_S x_S
+    n_iter: int
+    idx: np.ndarray          # [n_iter] atom taken at step t
+    gap: np.ndarray          # [n_iter] relative top-two gap of |c| on the oracle's own r
+    rnorm: np.ndarray        # [n_iter+1]
+    argmax_ref: np.ndarray   # [n_iter] the oracle's own argmax (differs from idx only in a forced replay)
+    cmax_ref: np.ndarray
+    c_at_idx: np.ndarray
+    status: int              # 0 ok, 2 = ended by a repeated atom / singular Gram matrix
+
+
+def omp(psi_t, y, eps: float, max_iter: int, idx_force=None, nthreads: int = 1) -> OMPResult:
+    """Orthogonal MP on the float32 dictionary; idx_force = teacher-forced replay of a given atom sequence."""
+    a, s, N, M, ld = _psi(psi_t)
+    if s != "f32":
+        raise TypeError("omp takes the float32 dictionary")
+    y = _f64(y)
+    force = None if idx_force is None else np.ascontiguousarray(idx_force, dtype=np.int32)
+    cap = max((force.size if force is not None else min(max_iter, N)), 1)
+    x = np.empty(M); r = np.empty(N); n_iter = C.c_int(0)
+    idx = np.empty(cap, dtype=np.int32); gap = np.empty(cap); rn = np.empty(cap + 1)
+    am = np.empty(cap, dtype=np.int32); cm = np.empty(cap); ci = np.empty(cap)
+    rc = _lib.oracle_omp_f32(_ptr(a), N, M, ld, _ptr(y), float(eps), int(max_iter),
+                             _ptr(force) if force is not None else None, int(force.size) if force is not None else 0,
+                             _ptr(x), _ptr(r), C.byref(n_iter), _ptr(idx), _ptr(gap), _ptr(rn), _ptr(am), _ptr(cm), _ptr(ci),
+                             nthreads)
+    if rc == 1:
+        raise ValueError("oracle_omp: invalid arguments")
+    t = n_iter.value
+    return OMPResult(x, r, t, idx[:t].copy(), gap[:t].copy(), rn[:t + 1].copy(), am[:t].copy(), cm[:t].copy(), ci[:t].copy(), rc)
 
 
 def encode_sparse(psi_t, idx, val) -> np.ndarray:

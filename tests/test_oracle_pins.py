@@ -443,3 +443,73 @@ def test_encode_sparse_pins():
     from paper_0809_1833_b200 import synth
     assert np.array_equal(y.astype(np.float32), synth.encode(psi, x, np.sort(idx))) or \
         np.allclose(y.astype(np.float32), synth.encode(psi, x, np.sort(idx)), rtol=2e-7)
+
+
+# ----------------------------------------------------------------------------- Orthogonal MP
+def _unit_rows(rng, M, N):
+    p = rng.standard_normal((M, N))
+    return (p / np.linalg.norm(p, axis=1, keepdims=True)).astype(np.float32)
+
+
+def test_omp_least_squares_and_orthogonality():
+    """After every step the coefficients are the least-squares solution on the selected atoms: they equal numpy's lstsq,
+    the residual is orthogonal to every selected atom, no atom is taken twice, ||r|| is non-increasing, and a K-sparse x
+    in the exact-recovery regime is recovered in exactly K steps (each step removes one atom for good)."""
+    rng = np.random.default_rng(11)
+    M, N, K = 300, 80, 7
+    psi = _unit_rows(rng, M, N)
+    P = psi.astype(np.float64)
+    s = rng.choice(M, K, replace=False)
+    x = np.zeros(M); x[s] = rng.standard_normal(K) + np.sign(rng.standard_normal(K))
+    y = P.T @ x
+    res = oracle.omp(psi, y, 1e-12, 40)
+    assert res.status == 0 and res.n_iter == K and set(res.idx.tolist()) == set(s.tolist())
+    assert len(set(res.idx.tolist())) == K and np.all(np.diff(res.rnorm) <= 1e-15)
+    assert np.allclose(res.x, x, atol=1e-13) and res.rnorm[-1] <= 1e-13 * res.rnorm[0]
+    for t in range(1, K + 1):                                               # every prefix is a least-squares fit
+        rp = oracle.omp(psi, y, 0.0, 0, idx_force=res.idx[:t])
+        S = res.idx[:t]
+        z = np.linalg.lstsq(P[S].T, y, rcond=None)[0]
+        assert np.allclose(rp.x[S], z, atol=1e-12) and not np.any(np.delete(rp.x, S))
+        assert np.max(np.abs(P[S] @ rp.r)) <= 1e-13 * np.linalg.norm(y)
+        assert np.allclose(rp.r, y - P[S].T @ z, atol=1e-12)
+
+
+def test_omp_equals_mp_on_orthonormal_dictionary_and_first_step():
+    """Orthonormal Psi: the refit changes nothing, OMP = MP (same atoms, same coefficients).  Any Psi: the first OMP step is
+    the first MP step divided by ||psi_i||^2 (= 1 for unit atoms)."""
+    N = 64
+    H = np.array([[1.0]])
+    while H.shape[0] < N:
+        H = np.block([[H, H], [H, -H]])
+    psi = (H / 8.0).astype(np.float32)
+    rng = np.random.default_rng(2)
+    s = rng.choice(N, 6, replace=False); x = np.zeros(N); x[s] = rng.standard_normal(6)
+    y = psi.astype(np.float64).T @ x
+    a = oracle.omp(psi, y, 1e-12, 30); b = oracle.mp(psi, y, 1e-12, 30)
+    assert a.n_iter == b.n_iter == 6 and np.array_equal(a.idx, b.idx) and np.allclose(a.x, b.x, atol=1e-15)
+    psi2 = _unit_rows(rng, 50, 20); y2 = rng.standard_normal(20)
+    a1 = oracle.omp(psi2, y2, 0.0, 1); b1 = oracle.mp(psi2, y2, 0.0, 1)
+    i = int(a1.idx[0])
+    assert i == int(b1.idx[0]) and a1.gap[0] == b1.gap[0]
+    nrm2 = float(np.sum(psi2[i].astype(np.float64) ** 2))
+    assert abs(a1.x[i] - b1.x[i] / nrm2) <= 1e-15
+
+
+def test_omp_two_atom_closed_form_and_edge_cases():
+    """Two atoms with coherence mu, y in their span: MP needs infinitely many steps (||r|| shrinks by |mu| each), OMP is exact
+    after two.  y = 0, T = 0, eps >= 1 give 0 steps; T is capped at N; a forced repeated atom ends the run (status 2)."""
+    mu = 0.9
+    psi = np.zeros((2, 4), np.float32); psi[0, 0] = 1.0; psi[1, 0] = mu; psi[1, 1] = np.sqrt(1 - np.float64(mu) ** 2)
+    P = psi.astype(np.float64)
+    y = 2.0 * P[0] - 1.5 * P[1]
+    res = oracle.omp(psi, y, 1e-13, 10)
+    assert res.n_iter == 2 and np.allclose(res.x, [2.0, -1.5], atol=1e-7) and res.rnorm[-1] <= 1e-7
+    assert oracle.mp(psi, y, 1e-6, 1000).n_iter > 50
+    assert oracle.omp(psi, np.zeros(4), 1e-5, 10).n_iter == 0
+    assert oracle.omp(psi, y, 1e-5, 0).n_iter == 0 and oracle.omp(psi, y, 1.0, 10).n_iter == 0
+    rng = np.random.default_rng(4)
+    psi3 = _unit_rows(rng, 40, 6)
+    assert oracle.omp(psi3, rng.standard_normal(6), 0.0, 100).n_iter <= 6
+    dup = oracle.omp(psi3, rng.standard_normal(6), 0.0, 0, idx_force=[3, 5, 3])
+    assert dup.status == 2 and dup.n_iter == 2
