@@ -143,6 +143,20 @@ MP_API mp_status mp_recover_f64(const double* psi_t, int N, int M, int64_t ld,
                          int* idx_trace, double* c_trace,
                          void* workspace, size_t workspace_bytes, void* stream);
 
+/* ---- Orthogonal Matching Pursuit (the paper's declared next target) -------------
+ * MP's selection (Eq. 9, Eq. 16: fp32 dots of the fp32 rounding of r, lowest index on ties) followed by a least-squares
+ * refit on the selected atoms, so that r = y - Psi_S x_S with x_S = argmin ||y - Psi_S z||_2 after every step.  The refit is
+ * a float64 QR factorisation grown by one column per iteration (Gram-Schmidt applied twice); x~ is obtained once, at the
+ * end, by back substitution.  Stop rule as MP; at most min(max_iter, N) atoms are taken; an atom that lies in the
+ * span of the selected ones ends the run.  Same layouts as mp_recover; idx_trace (nullable) receives the atoms in order.
+ * Runs as a stream of small kernels (the stop flag stays on the device; the host polls it every "chunk" iterations).
+ * Workspace: mp_workspace_bytes_omp(N, M, max_iter) bytes (dominated by the 8 * min(max_iter, N) * N byte basis). */
+MP_API size_t mp_workspace_bytes_omp(int N, int M, int max_iter);
+MP_API mp_status mp_recover_omp(const float* psi_t, int N, int M, int64_t ld,
+                         const float* y, float eps, int max_iter,
+                         float* x, float* r, int* n_iter, int* idx_trace,
+                         void* workspace, size_t workspace_bytes, void* stream);
+
 /* Description of the last error on this thread ("" if none).  Static storage, never NULL. */
 MP_API const char* mp_last_error(void);
 

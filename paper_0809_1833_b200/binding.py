@@ -64,6 +64,10 @@ lib.mp_normalize_columns_f64.restype = _i
 lib.mp_normalize_columns_f64.argtypes = [_vp, _i, _i, _i64, _vp, _vp]
 lib.mp_recover_f64.restype = _i
 lib.mp_recover_f64.argtypes = [_vp, _i, _i, _i64, _vp, C.c_double, _i, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]
+lib.mp_workspace_bytes_omp.restype = _sz
+lib.mp_workspace_bytes_omp.argtypes = [_i, _i, _i]
+lib.mp_recover_omp.restype = _i
+lib.mp_recover_omp.argtypes = [_vp, _i, _i, _i64, _vp, _f, _i, _vp, _vp, _vp, _vp, _vp, _sz, _vp]
 lib.mp_last_error.restype = C.c_char_p
 lib.mp_last_error.argtypes = []
 lib.mp_set_int.restype = _i
@@ -291,6 +295,29 @@ def mp_recover_f64(psi_t: torch.Tensor, y: torch.Tensor, eps: float, max_iter: i
                                   idx_trace.data_ptr() if trace else None, c_trace.data_ptr() if trace else None,
                                   base + off, workspace.numel() - off, _stream_ptr(stream)))
     return Recovered(x, r, n_iter, idx_trace, c_trace, workspace)
+
+
+def mp_recover_omp(psi_t: torch.Tensor, y: torch.Tensor, eps: float, max_iter: int, *, trace: bool = False,
+                   workspace=None, stream=None) -> Recovered:
+    """Orthogonal MP: MP's selection + least-squares refit; outputs are device tensors."""
+    p, N, M, ld = _dict_args(psi_t)
+    dev = psi_t.device
+    if y.numel() != N:
+        raise ValueError("y must have N elements")
+    x = torch.empty(M, dtype=torch.float32, device=dev)
+    r = torch.empty(N, dtype=torch.float32, device=dev)
+    n_iter = torch.empty(1, dtype=torch.int32, device=dev)
+    idx_trace = torch.empty(max(min(max_iter, N), 1), dtype=torch.int32, device=dev) if trace else None
+    need = lib.mp_workspace_bytes_omp(N, M, int(max_iter))
+    if workspace is None:
+        workspace = torch.empty(need + 256, dtype=torch.uint8, device=dev)
+    base = workspace.data_ptr()
+    off = (-base) % 256
+    with torch.cuda.device(dev):
+        _check(lib.mp_recover_omp(p, N, M, ld, _dev(y, torch.float32, "y"), float(eps), int(max_iter),
+                                  x.data_ptr(), r.data_ptr(), n_iter.data_ptr(), idx_trace.data_ptr() if trace else None,
+                                  base + off, workspace.numel() - off, _stream_ptr(stream)))
+    return Recovered(x, r, n_iter, idx_trace, None, workspace)
 
 
 def _host(t: torch.Tensor, dtype, what: str):

@@ -65,6 +65,11 @@ bool persistent_supported(int N, int M);
 mp_status launch_recover_persistent_ldg(const RecoverArgs& a, const Workspace& ws, cudaStream_t stream);
 bool persistent_ldg_supported(int N, int M);
 mp_status launch_recover_streamloop(const RecoverArgs& a, const Workspace& ws, cudaStream_t stream);
+// control-block slots of the stream-loop kernels (unsigned long long each) and its fused correlate+argmax launch,
+// shared with the Orthogonal MP loop (mp_omp.cu)
+enum { kCtrKey = 1, kCtrDone = 4, kCtrT = 5, kCtrYY = 6, kCtrRR = 7 };
+mp_status launch_sl_correlate_argmax(const float* psi_t, int N, int M, int64_t ld, const float* r32, unsigned long long* ctrl,
+                                     int blocks, cudaStream_t stream);
 
 struct BatchedArgs {
     const float* psi_t; int N, M; int64_t ld;

@@ -7,8 +7,6 @@
 
 namespace mp {
 
-// ctrl slots (unsigned long long each)
-enum { kCtrKey = 1, kCtrDone = 4, kCtrT = 5, kCtrYY = 6, kCtrRR = 7 };
 
 constexpr int kSLThreads = 1024;
 
@@ -131,6 +129,15 @@ sl_finish_kernel(int N, int M, const double* x64, const double* r64, const unsig
     for (int m = blockIdx.x * blockDim.x + threadIdx.x; m < M; m += gridDim.x * blockDim.x) x[m] = (float)x64[m];
     for (int n = blockIdx.x * blockDim.x + threadIdx.x; n < N; n += gridDim.x * blockDim.x) r[n] = (float)r64[n];
     if (blockIdx.x == 0 && threadIdx.x == 0) *n_iter = (int)ctrl[kCtrT];
+}
+
+mp_status launch_sl_correlate_argmax(const float* psi_t, int N, int M, int64_t ld, const float* r32, unsigned long long* ctrl,
+                                     int blocks, cudaStream_t stream)
+{
+    sl_correlate_argmax_kernel<<<blocks, 256, 0, stream>>>(psi_t, N, M, ld, r32, ctrl);
+    MP_CUDA(cudaGetLastError());
+    count_launch();
+    return MP_OK;
 }
 
 mp_status launch_recover_streamloop(const RecoverArgs& a, const Workspace& ws, cudaStream_t stream)
