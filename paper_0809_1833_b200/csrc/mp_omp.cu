@@ -80,37 +80,61 @@ omp_init_kernel(const float* __restrict__ y, int N, int Nr, float eps, int T, Om
     }
 }
 
-// h_j = <q_j, w> for j < t, one warp per basis vector.  pass 0: w = psi_i (the atom just selected); pass 1: w = ws.w.
+// h_j = <q_j, w> for j < t, one CTA of 8 warps per basis vector (fixed-order block sum).
+// pass 0: w = psi_i (the atom just selected); pass 1: w = ws.w.
 __global__ void __launch_bounds__(256)
 omp_hdots_kernel(const float* __restrict__ psi_t, int N, int Nr, int64_t ld, int pass, OmpWs ws)
 {
     if (ws.ctrl[kCtrDone]) return;
     const int t = (int)ws.ctrl[kCtrT];
-    const int j = blockIdx.x * 8 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+    const int j = blockIdx.x;
     if (j >= t) return;
+    __shared__ double part[8];
     const double* q = ws.Q + (size_t)j * Nr;
-    double s = 0.0;
+    double s0 = 0.0, s1 = 0.0;
     if (pass == 0) {
         const float* psi_i = psi_t + (int64_t)key_index(ws.ctrl[kCtrKey]) * ld;
-        for (int n = lane; n < N; n += 32) s += q[n] * (double)__ldg(psi_i + n);
+        int n = threadIdx.x;
+        for (; n + 256 < N; n += 512) { s0 += q[n] * (double)__ldg(psi_i + n); s1 += q[n + 256] * (double)__ldg(psi_i + n + 256); }
+        if (n < N) s0 += q[n] * (double)__ldg(psi_i + n);
     } else {
-        for (int n = lane; n < N; n += 32) s += q[n] * ws.w[n];
+        int n = threadIdx.x;
+        for (; n + 256 < N; n += 512) { s0 += q[n] * ws.w[n]; s1 += q[n + 256] * ws.w[n + 256]; }
+        if (n < N) s0 += q[n] * ws.w[n];
     }
-    s = warp_sum(s);
-    if (lane == 0) ws.h[j] = s;
+    const double s = warp_sum(s0 + s1);
+    if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) ws.h[j] = ((part[0] + part[1]) + (part[2] + part[3])) + ((part[4] + part[5]) + (part[6] + part[7]));
 }
 
-// w <- w - sum_{j<t} h_j q_j (ascending j), one thread per component; R[j][t] collects h_j of both passes.
+// w <- w - sum_{j<t} h_j q_j.  A CTA owns 32 components; its 8 warps take the basis vectors j = warp, warp + 8, ... and
+// their partial sums are added in warp order (fixed order).  R[j][t] collects h_j of both passes.
 __global__ void __launch_bounds__(256)
 omp_waxpy_kernel(const float* __restrict__ psi_t, int N, int Nr, int64_t ld, int T, int pass, OmpWs ws)
 {
     if (ws.ctrl[kCtrDone]) return;
     const int t = (int)ws.ctrl[kCtrT];
-    const int n = blockIdx.x * blockDim.x + threadIdx.x;
+    __shared__ double part[8][32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int n = blockIdx.x * 32 + lane;
+    double a0 = 0.0, a1 = 0.0;
     if (n < N) {
-        double v = pass == 0 ? (double)__ldg(psi_t + (int64_t)key_index(ws.ctrl[kCtrKey]) * ld + n) : ws.w[n];
-        for (int j = 0; j < t; j++) v -= ws.h[j] * ws.Q[(size_t)j * Nr + n];
-        ws.w[n] = v;
+        int j = warp;
+        for (; j + 8 < t; j += 16) {
+            a0 += ws.h[j] * ws.Q[(size_t)j * Nr + n];
+            a1 += ws.h[j + 8] * ws.Q[(size_t)(j + 8) * Nr + n];
+        }
+        if (j < t) a0 += ws.h[j] * ws.Q[(size_t)j * Nr + n];
+    }
+    part[warp][lane] = a0 + a1;
+    __syncthreads();
+    if (warp == 0 && n < N) {
+        double sum = 0.0;
+#pragma unroll
+        for (int w8 = 0; w8 < 8; w8++) sum += part[w8][lane];
+        const double v0 = pass == 0 ? (double)__ldg(psi_t + (int64_t)key_index(ws.ctrl[kCtrKey]) * ld + n) : ws.w[n];
+        ws.w[n] = v0 - sum;
     }
     if (blockIdx.x == 0)
         for (int j = threadIdx.x; j < t; j += blockDim.x) {
@@ -233,10 +257,10 @@ MP_API mp_status mp_recover_omp(const float* psi_t, int N, int M, int64_t ld,
         for (int k = 0; k < n; k++) {
             st = launch_sl_correlate_argmax(psi_t, N, M, ld, ws.r32, ws.ctrl, blocks, s);
             if (st != MP_OK) return st;
-            const int hb = (done_iters + k + 7) / 8;    // at most done_iters + k basis vectors exist at this iteration
+            const int hb = done_iters + k;              // at most done_iters + k basis vectors exist at this iteration
             for (int pass = 0; pass < 2; pass++) {
                 if (hb > 0) omp_hdots_kernel<<<hb, 256, 0, s>>>(psi_t, N, Nr, ld, pass, ws);
-                omp_waxpy_kernel<<<(N + 255) / 256, 256, 0, s>>>(psi_t, N, Nr, ld, Tld, pass, ws);
+                omp_waxpy_kernel<<<(N + 31) / 32, 256, 0, s>>>(psi_t, N, Nr, ld, Tld, pass, ws);
             }
             omp_finalize_kernel<<<1, kOmpThreads, 0, s>>>(N, Nr, eps, T, Tld, idx_trace, ws);
             count_launch(hb > 0 ? 5 : 3);

@@ -61,6 +61,17 @@ sl_correlate_argmax_kernel(const float* __restrict__ psi_t, int N, int M, int64_
         const float4* row4 = reinterpret_cast<const float4*>(row);
         float a0 = 0.f, a1 = 0.f;
         int j = lane;
+        for (; j + 224 < n4; j += 256) {                                     // 8 independent 16-byte loads in flight per lane
+            float4 p[8];
+#pragma unroll
+            for (int u = 0; u < 8; u++) p[u] = __ldg(row4 + j + 32 * u);
+#pragma unroll
+            for (int u = 0; u < 8; u += 2) {
+                const float4 u0 = r4[j + 32 * u], u1 = r4[j + 32 * u + 32];
+                a0 = fmaf(p[u].x, u0.x, a0); a0 = fmaf(p[u].y, u0.y, a0); a0 = fmaf(p[u].z, u0.z, a0); a0 = fmaf(p[u].w, u0.w, a0);
+                a1 = fmaf(p[u + 1].x, u1.x, a1); a1 = fmaf(p[u + 1].y, u1.y, a1); a1 = fmaf(p[u + 1].z, u1.z, a1); a1 = fmaf(p[u + 1].w, u1.w, a1);
+            }
+        }
         for (; j + 32 < n4; j += 64) {
             const float4 p = __ldg(row4 + j), q = __ldg(row4 + j + 32);
             const float4 u = r4[j], v = r4[j + 32];
