@@ -59,3 +59,32 @@ def test_argument_errors_are_detected_before_any_cuda_call():
     assert g(ok_ptr, 8, 8, 8, ok_ptr, 4, 2, 0.1, 1, ok_ptr, ok_ptr, ok_ptr, ok_ptr, 1 << 20, None) == 1          # ldy < N
     assert lib.mp_normalize_columns(None, 8, 8, 8, None, None) == 1
     assert lib.mp_last_error() != b""
+
+
+def test_argument_errors_of_the_widened_entry_points():
+    """encode / score / float64 / Orthogonal MP / batched correlation: validation happens on the host before any CUDA call."""
+    from paper_0809_1833_b200.binding import lib
+    ok = C.c_void_p(4096)
+    assert lib.mp_encode_sparse(None, 8, 8, 8, ok, ok, 2, ok, None) == 1
+    assert lib.mp_encode_sparse(ok, 8, 8, 8, None, ok, 2, ok, None) == 1                      # K > 0 needs idx
+    assert lib.mp_encode_sparse(ok, 8, 8, 8, ok, ok, -1, ok, None) == 1
+    assert lib.mp_reconstruction_error(ok, ok, 0, ok, None) == 1
+    assert lib.mp_reconstruction_error(ok, ok, 8, C.c_void_p(4100), None) == 1                # err_pct alignment
+    f = lib.mp_recover_f64
+    assert f(None, 8, 8, 8, ok, 0.1, 1, ok, ok, ok, None, None, ok, 1 << 20, None) == 1
+    assert f(ok, 8, 8, 7, ok, 0.1, 1, ok, ok, ok, None, None, ok, 1 << 20, None) == 1           # ld < N
+    assert f(ok, 7, 8, 7, ok, 0.1, 1, ok, ok, ok, None, None, ok, 1 << 20, None) == 1           # ld odd
+    assert f(ok, 8, 8, 8, ok, -0.1, 1, ok, ok, ok, None, None, ok, 1 << 20, None) == 1
+    assert f(ok, 8, 8, 8, ok, 0.1, 1, ok, ok, ok, None, None, ok, 16, None) == 4
+    assert lib.mp_workspace_bytes_f64(0, 8) == 0 and lib.mp_workspace_bytes_f64(8, 8) >= 256 + 64
+    g = lib.mp_recover_omp
+    assert g(None, 8, 8, 8, ok, 0.1, 1, ok, ok, ok, None, ok, 1 << 20, None) == 1
+    assert g(ok, 8, 8, 6, ok, 0.1, 1, ok, ok, ok, None, ok, 1 << 20, None) == 1               # ld < N
+    assert g(ok, 8, 8, 8, ok, 0.1, -1, ok, ok, ok, None, ok, 1 << 20, None) == 1
+    assert g(ok, 8, 8, 8, ok, 0.1, 4, ok, ok, ok, None, ok, 16, None) == 4
+    a = lib.mp_workspace_bytes_omp(4096, 16384, 512)
+    assert a >= 8 * 512 * 4096 and lib.mp_workspace_bytes_omp(4096, 16384, 10 ** 6) == lib.mp_workspace_bytes_omp(4096, 16384, 4096)
+    h = lib.mp_correlate_batched
+    assert h(ok, 8, 8, 8, ok, 8, 65, ok, ok, 1 << 20, None) == 1                              # B > 64
+    assert h(ok, 8, 8, 8, ok, 8, 2, ok, ok, 16, None) == 4
+    assert lib.mp_correlate_batched_workspace_bytes(8, 8, 65) == 0
