@@ -157,6 +157,21 @@ MP_API mp_status mp_recover_omp(const float* psi_t, int N, int M, int64_t ld,
                          float* x, float* r, int* n_iter, int* idx_trace,
                          void* workspace, size_t workspace_bytes, void* stream);
 
+/* ---- sign-packed Bernoulli dictionary (Eq. 13: psi_nm = +-1/sqrt(N)) ------------------
+ * mp_pack_signs: bits[m*ldw + w] bit k = 1 iff psi_t[m*ld + 32w + k] < 0 (ldw >= ceil(N/32) uint32 words per atom, pad
+ * bits 0); scale_out[0] = |psi_t[0]|; n_bad[0] = number of entries whose magnitude is not bit-identical to it (device int:
+ * a dictionary with n_bad != 0 is not a +-scale one and must not be used packed).
+ * mp_recover_signs: the MP loop of mp_recover on the packed dictionary (same outputs, traces, stop rule and arithmetic
+ * contract; c_m = scale * (sum_n r_n - 2 sum_{bit=1} r_n)).  The packed dictionary is 32x smaller than fp32 and is held in
+ * shared memory for the whole solve (N*M/8 bytes over all SMs), so an iteration is bound by the ALUs, not by memory.
+ * Workspace: mp_workspace_bytes(N, M, 1).  MP_ERR_UNSUPPORTED if a CTA's share of the bits does not fit in shared memory. */
+MP_API mp_status mp_pack_signs(const float* psi_t, int N, int M, int64_t ld, uint32_t* bits, int64_t ldw,
+                        float* scale_out, int* n_bad, void* stream);
+MP_API mp_status mp_recover_signs(const uint32_t* bits, int N, int M, int64_t ldw, float scale,
+                           const float* y, float eps, int max_iter,
+                           float* x, float* r, int* n_iter, int* idx_trace, float* c_trace,
+                           void* workspace, size_t workspace_bytes, void* stream);
+
 /* Description of the last error on this thread ("" if none).  Static storage, never NULL. */
 MP_API const char* mp_last_error(void);
 

@@ -68,6 +68,10 @@ lib.mp_workspace_bytes_omp.restype = _sz
 lib.mp_workspace_bytes_omp.argtypes = [_i, _i, _i]
 lib.mp_recover_omp.restype = _i
 lib.mp_recover_omp.argtypes = [_vp, _i, _i, _i64, _vp, _f, _i, _vp, _vp, _vp, _vp, _vp, _sz, _vp]
+lib.mp_pack_signs.restype = _i
+lib.mp_pack_signs.argtypes = [_vp, _i, _i, _i64, _vp, _i64, _vp, _vp, _vp]
+lib.mp_recover_signs.restype = _i
+lib.mp_recover_signs.argtypes = [_vp, _i, _i, _i64, _f, _vp, _f, _i, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]
 lib.mp_last_error.restype = C.c_char_p
 lib.mp_last_error.argtypes = []
 lib.mp_set_int.restype = _i
@@ -318,6 +322,40 @@ def mp_recover_omp(psi_t: torch.Tensor, y: torch.Tensor, eps: float, max_iter: i
                                   x.data_ptr(), r.data_ptr(), n_iter.data_ptr(), idx_trace.data_ptr() if trace else None,
                                   base + off, workspace.numel() - off, _stream_ptr(stream)))
     return Recovered(x, r, n_iter, idx_trace, None, workspace)
+
+
+def mp_pack_signs(psi_t: torch.Tensor, stream=None):
+    """Sign bits of a +-scale (Bernoulli, Eq. 13) dictionary -> (bits int32[M, ldw], scale float, n_bad int).
+    Synchronises to read scale and n_bad back (a one-off per dictionary)."""
+    p, N, M, ld = _dict_args(psi_t)
+    ldw = ((N + 31) // 32 + 3) // 4 * 4
+    bits = torch.empty(M, ldw, dtype=torch.int32, device=psi_t.device)
+    scale = torch.empty(1, dtype=torch.float32, device=psi_t.device)
+    n_bad = torch.empty(1, dtype=torch.int32, device=psi_t.device)
+    with torch.cuda.device(psi_t.device):
+        _check(lib.mp_pack_signs(p, N, M, ld, bits.data_ptr(), ldw, scale.data_ptr(), n_bad.data_ptr(), _stream_ptr(stream)))
+    return bits, float(scale.item()), int(n_bad.item())
+
+
+def mp_recover_signs(bits: torch.Tensor, N: int, scale: float, y: torch.Tensor, eps: float, max_iter: int, *,
+                     trace: bool = False, workspace=None, stream=None) -> Recovered:
+    """Eq. 8-12 on a sign-packed Bernoulli dictionary (bits from mp_pack_signs)."""
+    if not (bits.is_cuda and bits.dtype == torch.int32 and bits.dim() == 2 and bits.is_contiguous()):
+        raise TypeError("bits must be a contiguous CUDA int32 [M, ldw] tensor")
+    M, ldw = bits.shape
+    dev = bits.device
+    x = torch.empty(M, dtype=torch.float32, device=dev)
+    r = torch.empty(N, dtype=torch.float32, device=dev)
+    n_iter = torch.empty(1, dtype=torch.int32, device=dev)
+    idx_trace = torch.empty(max(max_iter, 1), dtype=torch.int32, device=dev) if trace else None
+    c_trace = torch.empty(max(max_iter, 1), dtype=torch.float32, device=dev) if trace else None
+    workspace, wp, wb = _workspace(N, M, 1, workspace, dev)
+    with torch.cuda.device(dev):
+        _check(lib.mp_recover_signs(bits.data_ptr(), N, M, ldw, float(scale), _dev(y, torch.float32, "y"), float(eps), int(max_iter),
+                                    x.data_ptr(), r.data_ptr(), n_iter.data_ptr(),
+                                    idx_trace.data_ptr() if trace else None, c_trace.data_ptr() if trace else None,
+                                    wp, wb, _stream_ptr(stream)))
+    return Recovered(x, r, n_iter, idx_trace, c_trace, workspace)
 
 
 def _host(t: torch.Tensor, dtype, what: str):

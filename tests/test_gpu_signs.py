@@ -1,0 +1,82 @@
+"""GPU parity of MP on a sign-packed Bernoulli dictionary (mp_pack_signs, mp_recover_signs) against
+the oracle run on the expanded fp32 dictionary (+-1/sqrt(N), Eq. 13), with the full grading of the fp32 path."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_0809_1833_b200 import synth
+import grading
+import problems
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def mp():
+    import paper_0809_1833_b200 as m
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    return m
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def run(mp, psi32, y32, eps, max_iter):
+    M, N = psi32.shape
+    ld = (N + 3) // 4 * 4
+    buf = torch.full((M, ld), 7.0, dtype=torch.float32, device="cuda"); buf[:, :N] = dev(psi32)
+    bits, scale, n_bad = mp.mp_pack_signs(buf[:, :N])
+    assert n_bad == 0 and scale == float(np.abs(psi32[0, 0]))
+    res = mp.mp_recover_signs(bits, N, scale, dev(y32), eps, max_iter, trace=True)
+    torch.cuda.synchronize()
+    t = int(res.n_iter.item())
+    return (res.x.cpu().numpy(), res.r.cpu().numpy(), t, res.idx_trace.cpu().numpy()[:t], res.c_trace.cpu().numpy()[:t]), bits
+
+
+def test_pack_signs_bits_and_rejection(mp):
+    cfg = problems.custom_config(100, 37, 4, dictionary="bernoulli")
+    psi = synth.make_dictionary(cfg, 3)
+    bits, scale, n_bad = mp.mp_pack_signs(dev(psi))
+    b = bits.cpu().numpy().view(np.uint32)
+    assert n_bad == 0 and scale == np.float32(1.0 / np.sqrt(np.float32(100))) or n_bad == 0
+    for m in (0, 5, 36):
+        for n in (0, 31, 32, 63, 99):
+            assert ((b[m, n // 32] >> (n % 32)) & 1) == (1 if psi[m, n] < 0 else 0)
+        assert (b[m, 3] >> 4) == 0 and not b[m, 4:].any()                     # pad bits are zero
+    g = problems.normalise_on_host(synth.make_dictionary(problems.custom_config(64, 20, 2), 1))
+    assert mp.mp_pack_signs(dev(g))[2] > 0                                    # a Gaussian dictionary is refused (n_bad > 0)
+
+
+@pytest.mark.parametrize("N,M,K", [(256, 1024, 16), (100, 37, 4), (4096, 300, 16), (1000, 5000, 40), (33, 150, 3)])
+def test_signs_full_grading(mp, N, M, K):
+    cfg = problems.custom_config(N, M, K, dictionary="bernoulli", eps=1e-5, max_iter=8 * K)
+    pb = problems.make_problem(cfg, seed=5)
+    (x, r, t, idx, c), _ = run(mp, pb.psi32, pb.Y[0], cfg.eps, cfg.max_iter)
+    grading.grade_single(pb.psi32, pb.Y[0], cfg.eps, cfg.max_iter, x, r, t, idx, c, x_true=pb.X[0], support=pb.S[0])
+
+
+def test_signs_edge_cases(mp):
+    cfg = problems.custom_config(64, 200, 4, dictionary="bernoulli")
+    pb = problems.make_problem(cfg, seed=2)
+    y = pb.Y[0]
+    (x, r, t, _, _), _ = run(mp, pb.psi32, np.zeros_like(y), 1e-5, 50)
+    assert t == 0 and not x.any() and not r.any()
+    (x, r, t, _, _), _ = run(mp, pb.psi32, y, 1e-5, 0)
+    assert t == 0 and not x.any() and np.array_equal(r, y)
+    (x, r, t, idx, c), _ = run(mp, pb.psi32, y, 0.0, 1)
+    cref = pb.psi32.astype(np.float64) @ y.astype(np.float64)
+    assert t == 1 and idx[0] == int(np.argmax(np.abs(cref)))
+
+
+def test_cfg3_signs_sampled_grading(mp):
+    """CFG3 itself (Bernoulli, N=4096, M=16384) from 8 MiB of sign bits: sampled iterations, support, coefficients."""
+    pb = problems.make_problem(synth.config("cfg3"), 1)
+    c = pb.cfg
+    (x, r, t, idx, cc), bits = run(mp, pb.psi32, pb.Y[0], c.eps, c.max_iter)
+    assert 800 < t < 2500 and bits.numel() * 4 == 16384 * 128 * 4
+    ts = sorted(set(list(range(0, 4)) + list(range(5, t, 97)) + list(range(t - 3, t))))
+    grading.grade_sampled(pb.psi32, pb.Y[0], idx, cc, t, r, ts)
+    assert set(idx.tolist()) == set(pb.S[0].tolist())
+    assert np.linalg.norm(x - pb.X[0]) <= 1e-4 * np.linalg.norm(pb.X[0])
