@@ -195,6 +195,7 @@ def main():
     ap.add_argument("--max-iter", type=int, default=None, help="override the config's iteration cap (profiling runs)")
     ap.add_argument("--f64", action="store_true", help="double-precision path (mp_recover_f64) on the same workload shape")
     ap.add_argument("--omp", action="store_true", help="Orthogonal MP (mp_recover_omp) on the same workload")
+    ap.add_argument("--signs", action="store_true", help="sign-packed Bernoulli dictionary (mp_recover_signs); Bernoulli configs only")
     ap.add_argument("--knob", action="append", default=[], metavar="NAME=VALUE", help="mp_set_int knob (profiling runs)")
     args = ap.parse_args()
     cfg = synth.config(args.config)
@@ -215,6 +216,8 @@ def main():
         return run_f64(args, cfg, torch, mp)
     if args.omp:
         return run_omp(args, cfg, torch, mp)
+    if args.signs:
+        return run_signs(args, cfg, torch, mp)
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
@@ -477,6 +480,55 @@ def run_omp(args, cfg, torch, mp):
                      "algorithmic_bytes_per_launch": alg_bytes, "kernel_ms": solve_ms,
                      "us_per_iteration": 1e3 * solve_ms / max(its, 1)},
         "cpu_baseline": cb, "e2e": None}))
+
+
+def run_signs(args, cfg, torch, mp):
+    """MP on the sign-packed Bernoulli dictionary (NEXT 4), 1 GPU.  One step = pack the signs + one whole solve.  The
+    iteration is ALU-bound: N*M conditional adds; peak = SMs x 128 fp32 lanes x max SM clock (B200_PROFILING.md counts)."""
+    if cfg.dictionary != "bernoulli":
+        raise SystemExit("--signs needs a Bernoulli configuration (cfg3)")
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(0)
+    N, M = cfg.N, cfg.M
+    psi_raw, X, S = build_problem(cfg, seed=1)
+    psi_d = torch.from_numpy(psi_raw).to(dev)
+    y_d = torch.from_numpy(synth.encode(psi_raw, X[0], S[0])).to(dev)
+    ws = torch.empty(mp.mp_workspace_bytes(N, M, 1) + 256, dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream()
+    for _ in range(args.warmup):
+        bits, scale, n_bad = mp.mp_pack_signs(psi_d); res = mp.mp_recover_signs(bits, N, scale, y_d, cfg.eps, cfg.max_iter, workspace=ws)
+    assert n_bad == 0
+    clocks = ClockSampler(0); clocks.start()
+    torch.cuda.synchronize()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2 * args.steps + 2)]
+    l0 = mp.mp_launch_count()
+    ev[0].record(stream)
+    for k in range(args.steps):
+        bits, scale, n_bad = mp.mp_pack_signs(psi_d)
+        ev[2 + 2 * k].record(stream)
+        res = mp.mp_recover_signs(bits, N, scale, y_d, cfg.eps, cfg.max_iter, workspace=ws)
+        ev[3 + 2 * k].record(stream)
+    ev[1].record(stream)
+    torch.cuda.synchronize()
+    clk = clocks.stop()
+    launches = mp.mp_launch_count() - l0
+    its = int(res.n_iter.item())
+    ms_total = ev[0].elapsed_time(ev[1])
+    solve_ms = float(np.mean([ev[2 + 2 * k].elapsed_time(ev[3 + 2 * k]) for k in range(args.steps)]))
+    sm = torch.cuda.get_device_properties(0).multi_processor_count
+    peak = sm * 128 * 1.965e9 / 1e12                       # T lane-ops/s
+    ach = its * float(N) * M / (solve_ms * 1e-3) / 1e12
+    print(json.dumps({
+        "metric": METRIC, "value": its * args.steps / (ms_total * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": workload_name(cfg) + ", dictionary as 1 sign bit per entry (N*M/8 = %.0f MiB, stationary in shared memory)" % (N * M / 8 / 2**20),
+                   "iterations_per_step": its, "step": "mp_pack_signs + mp_recover_signs (whole solve to the eps stop)", "parallelism": "1 GPU"},
+        "time_to_recovery_ms": solve_ms, "gpu_launches": int(launches), "clocks": clk,
+        "roofline": {"bound": "alu", "achieved": ach, "peak": peak, "unit": "T conditional adds/s", "frac": ach / peak, "traffic": None,
+                     "peak_source": "%d SMs x 128 fp32 lanes x 1.965 GHz, one lane-op per dictionary entry (a test plus an add is two)" % sm,
+                     "kernel": "mp_persistent_signs_kernel", "kernel_ms": solve_ms, "us_per_iteration": 1e3 * solve_ms / max(its, 1)},
+        "cpu_baseline": None, "e2e": None}))
 
 
 def mp_kernel_name(mp):
