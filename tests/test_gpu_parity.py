@@ -113,6 +113,17 @@ def test_ragged_shapes_full_grading(mp, N, M, K, ld, algo):
     grading.grade_single(pb.psi32, pb.Y[0], cfg.eps, cfg.max_iter, x, r, t, idx, cc)
 
 
+@pytest.mark.parametrize("N,M,K", [(20000, 64, 8), (16, 200000, 4), (19000, 160, 6), (3, 100000, 1)])
+def test_extreme_aspect_ratios_auto_dispatch(mp, N, M, K):
+    """Shapes at the edges of the kernels' plans under algo = auto: a residual too long for shared memory (stream loop),
+    a very long residual that still fits, and very many very short atoms."""
+    cfg = problems.custom_config(N, M, K, eps=1e-4, max_iter=4 * K + 2)
+    pb = problems.make_problem(cfg, seed=8)
+    x, r, t, idx, cc = run_single(mp, pb.psi32, pb.Y[0], cfg.eps, cfg.max_iter, 0)
+    grading.grade_single(pb.psi32, pb.Y[0], cfg.eps, cfg.max_iter, x, r, t, idx, cc)
+    assert mp.mp_get_int("info_algo") == (2 if N == 20000 else 3)
+
+
 # ------------------------------------------------------------------------------------------ edge / degenerate cases
 @pytest.mark.parametrize("algo", ALGOS)
 def test_edge_cases(mp, algo):
