@@ -149,7 +149,9 @@ MP_API mp_status mp_recover_f64(const double* psi_t, int N, int M, int64_t ld,
  * a float64 QR factorisation grown by one column per iteration (Gram-Schmidt applied twice); x~ is obtained once, at the
  * end, by back substitution.  Stop rule as MP; at most min(max_iter, N) atoms are taken; an atom that lies in the
  * span of the selected ones ends the run.  Same layouts as mp_recover; idx_trace (nullable) receives the atoms in order.
- * Runs as a stream of small kernels (the stop flag stays on the device; the host polls it every "chunk" iterations).
+ * Runs as one persistent cooperative kernel when the orthonormal basis, sliced by components over the CTAs, fits in shared
+ * memory (knob "omp_algo": 0 = auto, 1 = that kernel or MP_ERR_UNSUPPORTED, 2 = stream loop), else as a stream of small
+ * kernels (the stop flag stays on the device; the host polls it every "chunk" iterations).
  * Workspace: mp_workspace_bytes_omp(N, M, max_iter) bytes (dominated by the 8 * min(max_iter, N) * N byte basis). */
 MP_API size_t mp_workspace_bytes_omp(int N, int M, int max_iter);
 MP_API mp_status mp_recover_omp(const float* psi_t, int N, int M, int64_t ld,

@@ -133,6 +133,8 @@ static int64_t* option_slot(const char* name)
     if (!strcmp(name, "batched_algo")) return &o.batched_algo;
     if (!strcmp(name, "batched_coop")) return &o.batched_coop;
     if (!strcmp(name, "info_algo")) return &o.info_algo;
+    if (!strcmp(name, "omp_algo")) return &o.omp_algo;
+    if (!strcmp(name, "info_omp_algo")) return &o.info_omp_algo;
     if (!strcmp(name, "info_tc_clusters")) return &o.info_tc_clusters;
     if (!strcmp(name, "info_tc_at")) return &o.info_tc_at;
     if (!strcmp(name, "info_tc_stages")) return &o.info_tc_stages;

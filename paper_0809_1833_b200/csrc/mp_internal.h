@@ -21,6 +21,7 @@ mp_status cuda_fail(cudaError_t e, const char* what);
 struct Options {
     int64_t algo = 0, warps = 0, slot_bytes = 0, depth = 0, grid = 0, chunk = 64;
     int64_t batched_algo = 0, batched_coop = 1;
+    int64_t omp_algo = 0, info_omp_algo = 0;   // Orthogonal MP: 0 auto, 1 persistent kernel, 2 stream loop; and the one last used
     int64_t info_algo = 0;             // kernel the last mp_recover call used (1, 2 or 3)
     int64_t info_tc_clusters = 0, info_tc_at = 0, info_tc_stages = 0;   // plan of the last batched tensor-core launch (read-only use)
 };

@@ -10,38 +10,28 @@
 // per iteration); the refit reads the t x N basis twice per iteration (16 t N bytes, L2-resident at these sizes).
 #include "mp_common.cuh"
 #include "mp_internal.h"
+#include "mp_omp.h"
 
 namespace mp {
 
 constexpr int kOmpThreads = 1024;
 
-struct OmpWs {
-    unsigned long long* ctrl;   // stream-loop control block (kCtr*)
-    double* r64;                // Nr
-    float* r32;                 // Nr
-    double* w;                  // Nr   the new direction being orthogonalised
-    double* h;                  // T    Q^T w of the current pass
-    double* z;                  // T    Q^T y
-    double* Rm;                 // T x T upper triangular, row-major
-    int* sel;                   // T    selected atoms in order
-    double* Q;                  // T x Nr orthonormal basis of span(Psi_S), row-major
-    size_t bytes;
-};
-
-static size_t omp_layout(int N, int T, void* base, OmpWs* ws)
+size_t omp_layout(int N, int T, void* base, OmpWs* ws)
 {
     const size_t Nr = (size_t)round_up(N, 128), Tr = (size_t)round_up(T > 0 ? T : 1, 32);
     size_t off = 0;
     char* b = static_cast<char*>(base);
     auto take = [&](size_t bytes) { size_t o = off; off = (off + bytes + 255) / 256 * 256; return o; };
     const size_t o_ctrl = take(256), o_r64 = take(8 * Nr), o_r32 = take(4 * Nr), o_w = take(8 * Nr), o_h = take(8 * Tr),
-                 o_z = take(8 * Tr), o_R = take(8 * Tr * Tr), o_sel = take(4 * Tr), o_Q = take(8 * Tr * Nr);
+                 o_z = take(8 * Tr), o_R = take(8 * Tr * Tr), o_sel = take(4 * Tr), o_Q = take(8 * Tr * Nr),
+                 o_hp = take(8 * Tr * kOmpMaxCtas), o_sc = take(8 * 2 * kOmpMaxCtas);
     if (ws) {
         ws->ctrl = reinterpret_cast<unsigned long long*>(b + o_ctrl);
         ws->r64 = reinterpret_cast<double*>(b + o_r64); ws->r32 = reinterpret_cast<float*>(b + o_r32);
         ws->w = reinterpret_cast<double*>(b + o_w); ws->h = reinterpret_cast<double*>(b + o_h);
         ws->z = reinterpret_cast<double*>(b + o_z); ws->Rm = reinterpret_cast<double*>(b + o_R);
         ws->sel = reinterpret_cast<int*>(b + o_sel); ws->Q = reinterpret_cast<double*>(b + o_Q);
+        ws->hpart = reinterpret_cast<double*>(b + o_hp); ws->scal = reinterpret_cast<double*>(b + o_sc);
         ws->bytes = off;
     }
     return off;
@@ -245,6 +235,20 @@ MP_API mp_status mp_recover_omp(const float* psi_t, int N, int M, int64_t ld,
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     const int Nr = round_up(N, 128), Tld = round_up(T > 0 ? T : 1, 32);
 
+    // omp_algo 0 = auto (the persistent kernel when the basis slices fit in shared memory), 1 = persistent or error,
+    // 2 = the stream loop below
+    const int64_t oalgo = options().omp_algo;
+    if (T > 0 && oalgo != 2 && (oalgo == 1 || omp_persistent_supported(N, M, T))) {
+        OmpArgs oa{psi_t, N, M, ld, y, eps, T, idx_trace};
+        st = launch_omp_persistent(oa, ws, s);
+        if (st != MP_OK) return st;
+        omp_finish_kernel<<<1, kOmpThreads, 0, s>>>(N, M, Tld, x, r, n_iter, ws);
+        MP_CUDA(cudaGetLastError());
+        count_launch();
+        options().info_omp_algo = 1;
+        return MP_OK;
+    }
+    options().info_omp_algo = 2;
     omp_init_kernel<<<1, kOmpThreads, 0, s>>>(y, N, Nr, eps, T, ws);
     MP_CUDA(cudaGetLastError());
     count_launch();

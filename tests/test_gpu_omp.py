@@ -25,13 +25,18 @@ def mp():
     assert torch.cuda.is_available(), "GPU tests need a CUDA device"
     yield m
     m.mp_set_int("chunk", 64)
+    m.mp_set_int("omp_algo", 0)
+
+
+OMP_ALGOS = [1, 2]        # 1 = one persistent kernel (basis slices stationary in shared memory), 2 = stream loop of small kernels
 
 
 def dev(a):
     return torch.from_numpy(np.ascontiguousarray(a)).cuda()
 
 
-def run(mp, psi32, y32, eps, max_iter, ld=None):
+def run(mp, psi32, y32, eps, max_iter, ld=None, algo=0):
+    mp.mp_set_int("omp_algo", algo)
     M, N = psi32.shape
     if ld is None:
         ld = (N + 3) // 4 * 4
@@ -73,44 +78,49 @@ def grade_omp(psi32, y32, eps, max_iter, x, r, t, idx, x_true=None, support=None
     return ref
 
 
+@pytest.mark.parametrize("algo", OMP_ALGOS)
 @pytest.mark.parametrize("seed", [1, 2, 3])
-def test_cfg1_omp_full_grading(mp, seed):
+def test_cfg1_omp_full_grading(mp, seed, algo):
     pb = problems.make_problem(synth.config("cfg1"), seed)
     c = pb.cfg
-    x, r, t, idx = run(mp, pb.psi32, pb.Y[0], c.eps, c.max_iter)
+    x, r, t, idx = run(mp, pb.psi32, pb.Y[0], c.eps, c.max_iter, algo=algo)
+    assert mp.mp_get_int("info_omp_algo") == algo
     ref = grade_omp(pb.psi32, pb.Y[0], c.eps, c.max_iter, x, r, t, idx, x_true=pb.X[0], support=pb.S[0])
     assert t <= c.K and ref.n_iter == t                                      # OMP: one step per atom of the support
 
 
 @pytest.mark.parametrize("N,M,K,ld", [(250, 1000, 10, None), (37, 5, 2, 40), (1, 3, 1, 4), (130, 149, 6, 256),
                                       (2052, 777, 20, None), (512, 4099, 24, None)])
-def test_ragged_shapes_omp(mp, N, M, K, ld):
+@pytest.mark.parametrize("algo", OMP_ALGOS)
+def test_ragged_shapes_omp(mp, N, M, K, ld, algo):
     cfg = problems.custom_config(N, M, K, eps=1e-4, max_iter=3 * K + 3)
     pb = problems.make_problem(cfg, seed=4)
-    x, r, t, idx = run(mp, pb.psi32, pb.Y[0], cfg.eps, cfg.max_iter, ld)
+    x, r, t, idx = run(mp, pb.psi32, pb.Y[0], cfg.eps, cfg.max_iter, ld, algo=algo)
     grade_omp(pb.psi32, pb.Y[0], cfg.eps, cfg.max_iter, x, r, t, idx)
 
 
-def test_edge_cases_omp(mp):
+@pytest.mark.parametrize("algo", OMP_ALGOS)
+def test_edge_cases_omp(mp, algo):
     pb = problems.make_problem(problems.custom_config(64, 200, 4), seed=2)
     y = pb.Y[0]
-    x, r, t, _ = run(mp, pb.psi32, np.zeros_like(y), 1e-5, 50)
+    x, r, t, _ = run(mp, pb.psi32, np.zeros_like(y), 1e-5, 50, algo=algo)
     assert t == 0 and not x.any() and not r.any()
-    x, r, t, _ = run(mp, pb.psi32, y, 1e-5, 0)
+    x, r, t, _ = run(mp, pb.psi32, y, 1e-5, 0, algo=0)
     assert t == 0 and not x.any() and np.array_equal(r.astype(np.float32), y)
-    x, r, t, _ = run(mp, pb.psi32, y, 1.0, 50)
+    x, r, t, _ = run(mp, pb.psi32, y, 1.0, 50, algo=algo)
     assert t == 0
     mp.mp_set_int("chunk", 3)                                                # several host polls
     pb2 = problems.make_problem(problems.custom_config(64, 200, 30), seed=3)
-    x, r, t, idx = run(mp, pb2.psi32, pb2.Y[0], 0.0, 20)                     # eps = 0: runs to max_iter
+    x, r, t, idx = run(mp, pb2.psi32, pb2.Y[0], 0.0, 20, algo=algo)          # eps = 0: runs to max_iter
     mp.mp_set_int("chunk", 64)
     assert t == 20
     grade_omp(pb2.psi32, pb2.Y[0], 0.0, 20, x, r, t, idx)
-    x, r, t, idx = run(mp, pb2.psi32, pb2.Y[0], 0.0, 1000)                   # capped at N atoms
+    x, r, t, idx = run(mp, pb2.psi32, pb2.Y[0], 0.0, 1000, algo=algo)        # capped at N atoms
     assert t <= 64
 
 
-def test_omp_equals_mp_on_orthonormal_dictionary(mp):
+@pytest.mark.parametrize("algo", OMP_ALGOS)
+def test_omp_equals_mp_on_orthonormal_dictionary(mp, algo):
     N = 256
     H = np.array([[1.0]])
     while H.shape[0] < N:
@@ -120,15 +130,16 @@ def test_omp_equals_mp_on_orthonormal_dictionary(mp):
     s = rng.choice(N, 12, replace=False)
     x_true = np.zeros(N); x_true[s] = rng.standard_normal(12)
     y = (psi.astype(np.float64).T @ x_true).astype(np.float32)
-    x, r, t, idx = run(mp, psi, y, 1e-6, 100)
+    x, r, t, idx = run(mp, psi, y, 1e-6, 100, algo=algo)
     assert t == 12 and list(idx) == list(s[np.argsort(-np.abs(x_true[s]), kind="stable")])
     assert np.allclose(x, x_true, atol=2e-7)
 
 
-def test_cfg2_size_omp(mp):
+@pytest.mark.parametrize("algo", OMP_ALGOS)
+def test_cfg2_size_omp(mp, algo):
     """N=2048, M=8192, K=128: OMP takes exactly the support in K steps; the replay grades every step."""
     pb = problems.make_problem(synth.config("cfg2"), 1)
     c = pb.cfg
-    x, r, t, idx = run(mp, pb.psi32, pb.Y[0], c.eps, 4 * c.K)
+    x, r, t, idx = run(mp, pb.psi32, pb.Y[0], c.eps, 4 * c.K, algo=algo)
     assert t == c.K and set(idx.tolist()) == set(pb.S[0].tolist())
     grade_omp(pb.psi32, pb.Y[0], c.eps, 4 * c.K, x, r, t, idx, x_true=pb.X[0], support=pb.S[0])
