@@ -24,7 +24,7 @@ size_t omp_layout(int N, int T, void* base, OmpWs* ws)
     auto take = [&](size_t bytes) { size_t o = off; off = (off + bytes + 255) / 256 * 256; return o; };
     const size_t o_ctrl = take(256), o_r64 = take(8 * Nr), o_r32 = take(4 * Nr), o_w = take(8 * Nr), o_h = take(8 * Tr),
                  o_z = take(8 * Tr), o_R = take(8 * Tr * Tr), o_sel = take(4 * Tr), o_Q = take(8 * Tr * Nr),
-                 o_hp = take(8 * Tr * kOmpMaxCtas), o_sc = take(8 * 2 * kOmpMaxCtas);
+                 o_hp = take(8 * Tr * kOmpMaxCtas), o_sc = take(8 * 4 * kOmpMaxCtas);
     if (ws) {
         ws->ctrl = reinterpret_cast<unsigned long long*>(b + o_ctrl);
         ws->r64 = reinterpret_cast<double*>(b + o_r64); ws->r32 = reinterpret_cast<float*>(b + o_r32);

@@ -17,7 +17,7 @@ struct OmpWs {
     int* sel;                   // T    selected atoms in order
     double* Q;                  // T x Nr orthonormal basis of span(Psi_S), row-major (stream loop only)
     double* hpart;              // kOmpMaxCtas x T per-CTA partial dots (persistent kernel)
-    double* scal;               // kOmpMaxCtas x 2 per-CTA partial ||w||^2, <w, r> (persistent kernel)
+    double* scal;               // kOmpMaxCtas x 4 per-CTA partial ||w||^2, <w, r>, ||psi_i||^2 (persistent kernel)
     size_t bytes;
 };
 

@@ -7,8 +7,8 @@
 //     barrier 1   winning key (as MP)
 //     partial h = Q_slice^T psi_i,slice -> global [cta][j]            barrier 2
 //     CTA j mod G adds the G partials of h_j in a fixed order           barrier 3
-//     w_slice = psi_i,slice - Q_slice h ; second pass: partial h'       barrier 4,  reduce, barrier 5
-//     w_slice -= Q_slice h' ; partial ||w||^2, <w, r> and the slice of w -> global                     barrier 6
+//     w_slice = psi_i,slice - Q_slice h ; partial ||w||^2, <w, r> and the slice of w -> global           barrier 4
+//     (a second Gram-Schmidt pass, three more barriers, only if ||w||^2 < ||psi_i||^2 / 2: the usual criterion)
 //     everybody: ||w||^2, <w, r> (fixed order), r <- r - (<w,r>/||w||^2) w on its own full copy of r, ||r||^2, stop test;
 //     q_t,slice = w_slice / ||w|| joins the CTA's basis slice.
 // R, z and the selected atoms go to the workspace; x~ is produced by the stream loop's back-substitution kernel.
@@ -228,40 +228,56 @@ mp_omp_persistent_kernel(const OmpPParams p)
         __syncthreads();
         const int i = key_index(*skey);
 
-        // ---------- refit: w <- psi_i - Q Q^T psi_i, twice -----------------------------------------------------------------------
+        // ---------- refit: w <- psi_i - Q Q^T psi_i -----------------------------------------------------------------------------
         const float* psi_i = p.psi_t + (int64_t)i * p.ld;
         if (tid < SL) wsl[tid] = (double)__ldg(psi_i + s0 + tid);
         __syncthreads();
+        // Gram-Schmidt with the usual reorthogonalisation criterion: a second pass only if the first one removed more
+        // than half of the atom's energy (||w||^2 < ||psi_i||^2 / 2); for incoherent atoms it almost never does.
+        double nrm2 = 0.0, zn = 0.0;
         for (int pass = 0; pass < 2; pass++) {
+            double pa = 0.0;
+            if (pass == 0 && warp == 0) {
+                for (int n = lane; n < SL; n += 32) pa += wsl[n] * wsl[n];
+                pa = warp_sum(pa);
+            }
             if (t > 0) {
                 partial_h(t);
-                grid_sync();                                                   // barriers 2 / 4
+                grid_sync();                                                   // partial dots out
                 reduce_h(t);
-                grid_sync();                                                   // barriers 3 / 5
+                grid_sync();                                                   // h reduced
                 subtract_projection(t, pass == 0);
             }
+            // ---------- ||w||^2, <w, r>, (||psi_i||^2) and the slice of w for everybody ------------------------------------
+            if (warp == 0) {
+                double pw = 0.0, pz = 0.0;
+                for (int n = lane; n < SL; n += 32) { pw += wsl[n] * wsl[n]; pz += wsl[n] * r64[s0 + n]; }
+                pw = warp_sum(pw);
+                pz = warp_sum(pz);
+                if (lane == 0) {
+                    ws.scal[4 * b] = pw; ws.scal[4 * b + 1] = pz;
+                    if (pass == 0) ws.scal[4 * b + 2] = pa;
+                }
+            }
+            if (tid < SL) ws.w[s0 + tid] = wsl[tid];
+            if (b == 0 && tid == 0 && pass == 0) st_relaxed_u64(ws.ctrl + 1 + ((t + 2) % 3), 0ull);   // key slot of t-1, reused at t+2
+            grid_sync();                                                       // exchange
+            if (warp == 0) {
+                double nw = 0.0, z1 = 0.0, aa = 0.0;
+                for (int c = lane; c < G; c += 32) {
+                    nw += __ldcg(ws.scal + 4 * c); z1 += __ldcg(ws.scal + 4 * c + 1); aa += __ldcg(ws.scal + 4 * c + 2);
+                }
+                nw = warp_sum(nw);
+                z1 = warp_sum(z1);
+                aa = warp_sum(aa);
+                if (lane == 0) { red[0] = nw; red[1] = z1; red[2] = aa; }
+            }
+            __syncthreads();
+            nrm2 = red[0]; zn = red[1];
+            const bool again = pass == 0 && t > 0 && nrm2 < 0.5 * red[2];
+            __syncthreads();
+            if (!again) break;
         }
-        // ---------- ||w||^2, <w, r>, and the slice of w for everybody ---------------------------------------------------------------
-        if (warp == 0) {
-            double pw = 0.0, pz = 0.0;
-            for (int n = lane; n < SL; n += 32) { pw += wsl[n] * wsl[n]; pz += wsl[n] * r64[s0 + n]; }
-            pw = warp_sum(pw);
-            pz = warp_sum(pz);
-            if (lane == 0) { ws.scal[2 * b] = pw; ws.scal[2 * b + 1] = pz; }
-        }
-        if (tid < SL) ws.w[s0 + tid] = wsl[tid];
-        if (b == 0 && tid == 0) st_relaxed_u64(ws.ctrl + 1 + ((t + 2) % 3), 0ull);   // key slot of iteration t-1, reused at t+2
-        grid_sync();                                                           // barrier 6
-        if (warp == 0) {
-            double nw = 0.0, zn = 0.0;
-            for (int c = lane; c < G; c += 32) { nw += __ldcg(ws.scal + 2 * c); zn += __ldcg(ws.scal + 2 * c + 1); }
-            nw = warp_sum(nw);
-            zn = warp_sum(zn);
-            if (lane == 0) { red[0] = nw; red[1] = zn; }
-        }
-        __syncthreads();
-        const double nrm2 = red[0], zn = red[1];
-        __syncthreads();
         if (!(nrm2 > 1e-20)) break;                                            // the atom lies in the span of the selected ones
         const double nrm = sqrt(nrm2), coef = zn / nrm2;
         if (tid < SL) Qs[(size_t)t * p.SLp + tid] = wsl[tid] / nrm;            // q_t joins the basis slice

@@ -143,3 +143,23 @@ def test_cfg2_size_omp(mp, algo):
     x, r, t, idx = run(mp, pb.psi32, pb.Y[0], c.eps, 4 * c.K, algo=algo)
     assert t == c.K and set(idx.tolist()) == set(pb.S[0].tolist())
     grade_omp(pb.psi32, pb.Y[0], c.eps, 4 * c.K, x, r, t, idx, x_true=pb.X[0], support=pb.S[0])
+
+
+@pytest.mark.parametrize("a", [2.0, 5.0])
+@pytest.mark.parametrize("algo", OMP_ALGOS)
+def test_coherent_dictionary_omp(mp, a, algo):
+    """Atoms share a strong common component (pairwise coherence a^2/(a^2+1) = 0.8 / 0.96): after the first pick the
+    Gram-Schmidt step removes more than half of every later atom, which is where a single pass loses orthogonality and the
+    persistent kernel's second pass has to run.  Same grading as everywhere: picks against the oracle's normal-equation OMP,
+    x = the least-squares solution on the selected set, r = y - Psi_S x_S."""
+    N, M, K = 300, 640, 8
+    rng = np.random.default_rng(11)
+    u = rng.standard_normal(N); u /= np.linalg.norm(u)
+    raw = (a * u[None, :] + rng.standard_normal((M, N)) / np.sqrt(N)).astype(np.float32)
+    psi32 = problems.normalise_on_host(raw)
+    s = rng.choice(M, K, replace=False)
+    x_true = np.zeros(M); x_true[s] = rng.standard_normal(K)
+    y = (psi32.astype(np.float64).T @ x_true).astype(np.float32)
+    x, r, t, idx = run(mp, psi32, y, 1e-5, 4 * K, algo=algo)
+    assert t >= 2
+    grade_omp(psi32, y, 1e-5, 4 * K, x, r, t, idx)
