@@ -539,7 +539,8 @@ def mp_kernel_name(mp):
             return ("mp_batched_tc_kernel (%d clusters x 4 CTAs, %d atoms/tile, %d stages)"
                     % (mp.mp_get_int("info_tc_clusters"), mp.mp_get_int("info_tc_at"), mp.mp_get_int("info_tc_stages")))
         return {1: "mp_persistent_kernel (TMA-staged)", 2: "stream loop",
-                3: "mp_persistent_ldg_kernel (register-streaming)"}[mp.mp_get_int("info_algo")]
+                3: "mp_persistent_ldg_kernel (register-streaming)",
+                4: "mp_many_kernel (one cluster, dictionary stationary in shared memory)"}[mp.mp_get_int("info_algo")]
     except Exception:
         return "?"
 

@@ -174,11 +174,34 @@ MP_API mp_status mp_recover_signs(const uint32_t* bits, int N, int M, int64_t ld
                            float* x, float* r, int* n_iter, int* idx_trace, float* c_trace,
                            void* workspace, size_t workspace_bytes, void* stream);
 
+/* ---- many independent small problems (the paper's Fig. 1 experiment) -----------------
+ * P problems of one shape (N, M), each with its OWN dictionary and measurement vector -- the (sigma, rho) phase diagram is
+ * 100 trials per cell at M = 1000 with a fresh Bernoulli dictionary per trial -- solved by one launch:
+ *   psi_t   in   problem q's dictionary starts at psi_t + q*problem_stride (floats; atom-major, row stride ld as above);
+ *                problem_stride = 0 means all P problems share ONE dictionary (then this equals mp_recover_batched)
+ *   Y       in   P x N, row stride ldy >= N (any; only 4-byte alignment is needed for Y, X, R here);   X out P x M;
+ *                R out P x N;   n_iter out P ints
+ *   idx_trace / c_trace   nullable, [q*ldt + t] for t < n_iter[q], ldt >= max_iter
+ * Problem q's result equals mp_recover on (dictionary q, Y[q]) under the same arithmetic contract.  One thread-block
+ * cluster (1-16 CTAs) owns a problem at a time: its dictionary is held in the cluster's shared memory for the whole solve
+ * when it fits (<= ~3.5 MB), else streamed from L2; the argmax is exchanged through distributed shared memory with one
+ * hardware cluster barrier per iteration; clusters draw problems from a device counter.  N > 2048 falls back to one
+ * single-signal solve after another.  Knobs: "many_cluster" (CTAs per problem, 0 = auto), "many_threads", "many_stat"
+ * (2 = never stationary).  Workspace: mp_workspace_bytes_many(N, M, P). */
+MP_API size_t mp_workspace_bytes_many(int N, int M, int P);
+MP_API mp_status mp_recover_many(const float* psi_t, int N, int M, int64_t ld, int64_t problem_stride,
+                          const float* Y, int64_t ldy, int P, float eps, int max_iter,
+                          float* X, float* R, int* n_iter,
+                          int* idx_trace, float* c_trace, int64_t ldt,
+                          void* workspace, size_t workspace_bytes, void* stream);
+
 /* Description of the last error on this thread ("" if none).  Static storage, never NULL. */
 MP_API const char* mp_last_error(void);
 
 /* Tuning / diagnostic knobs (process-wide, not part of the method).  Unknown name -> MP_ERR_INVALID_ARG.
- *   "algo"          0 = auto (default: 3 if it fits, else 1, else 2), 1 = persistent cooperative kernel fed by TMA bulk
+ *   "algo"          0 = auto (default: 4 if one cluster can hold the dictionary in shared memory -- 4NM <= ~3.4 MB, N <= 2048 --
+ *                   else 3 if it fits, else 1, else 2), 4 = the cluster kernel of mp_recover_many with P = 1 (N <= 2048),
+ *                   1 = persistent cooperative kernel fed by TMA bulk
  *                   copies through shared memory, 2 = stream loop of small kernels (general fallback; synchronises the
  *                   host every "chunk" iterations to read the stop flag), 3 = persistent cooperative kernel that streams
  *                   the dictionary into registers with 128-bit loads

@@ -72,6 +72,10 @@ lib.mp_pack_signs.restype = _i
 lib.mp_pack_signs.argtypes = [_vp, _i, _i, _i64, _vp, _i64, _vp, _vp, _vp]
 lib.mp_recover_signs.restype = _i
 lib.mp_recover_signs.argtypes = [_vp, _i, _i, _i64, _f, _vp, _f, _i, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]
+lib.mp_workspace_bytes_many.restype = _sz
+lib.mp_workspace_bytes_many.argtypes = [_i, _i, _i]
+lib.mp_recover_many.restype = _i
+lib.mp_recover_many.argtypes = [_vp, _i, _i, _i64, _i64, _vp, _i64, _i, _f, _i, _vp, _vp, _vp, _vp, _vp, _i64, _vp, _sz, _vp]
 lib.mp_last_error.restype = C.c_char_p
 lib.mp_last_error.argtypes = []
 lib.mp_set_int.restype = _i
@@ -212,6 +216,44 @@ def mp_recover_batched(psi_t: torch.Tensor, Y: torch.Tensor, eps: float, max_ite
             _dev(idx_trace, torch.int32, "idx_trace") if idx_trace is not None else None,
             _dev(c_trace, torch.float32, "c_trace") if c_trace is not None else None, ldt,
             wp, wb, _stream_ptr(stream)))
+    return Recovered(X, R, n_iter, idx_trace, c_trace, workspace)
+
+
+def mp_recover_many(psi_t: torch.Tensor, Y: torch.Tensor, eps: float, max_iter: int, *, trace: bool = False,
+                    workspace=None, stream=None) -> Recovered:
+    """P independent problems of one shape (the paper's Fig. 1 workload): psi_t[P, M, N] (or [M, N]: one shared
+    dictionary), Y[P, N] -> X[P, M], R[P, N], n_iter[P] (+ traces [P, max_iter]); one thread-block cluster per problem."""
+    if not (psi_t.is_cuda and psi_t.dtype == torch.float32 and psi_t.dim() in (2, 3) and (psi_t.shape[-1] == 1 or psi_t.stride(-1) == 1)):
+        raise TypeError("psi_t must be a CUDA float32 [P, M, N] (or [M, N]) tensor with unit stride along N")
+    M, N = psi_t.shape[-2:]
+    dev = psi_t.device
+    if not (Y.is_cuda and Y.dtype == torch.float32 and Y.dim() == 2 and Y.shape[1] == N and (N == 1 or Y.stride(1) == 1)):
+        raise TypeError("Y must be a CUDA float32 [P, N] tensor with unit stride along N")
+    P = Y.shape[0]
+    ld = psi_t.stride(-2) if M > 1 else max(psi_t.stride(-2), N)
+    if psi_t.dim() == 3:
+        if psi_t.shape[0] != P:
+            raise ValueError("psi_t[P, M, N] and Y[P, N] disagree on P")
+        pstride = psi_t.stride(0) if P > 1 else max(psi_t.stride(0), M * ld)
+    else:
+        pstride = 0
+    ldy = Y.stride(0) if P > 1 else max(Y.stride(0), N)
+    X = torch.empty(P, M, dtype=torch.float32, device=dev)
+    R = torch.empty(P, N, dtype=torch.float32, device=dev)
+    n_iter = torch.empty(P, dtype=torch.int32, device=dev)
+    ldt = max(max_iter, 1)
+    idx_trace = torch.empty(P, ldt, dtype=torch.int32, device=dev) if trace else None
+    c_trace = torch.empty(P, ldt, dtype=torch.float32, device=dev) if trace else None
+    need = lib.mp_workspace_bytes_many(N, M, P)
+    if workspace is None:
+        workspace = torch.empty(need + 256, dtype=torch.uint8, device=dev)
+    base = workspace.data_ptr()
+    off = (-base) % 256
+    with torch.cuda.device(dev):
+        _check(lib.mp_recover_many(psi_t.data_ptr(), N, M, ld, pstride, Y.data_ptr(), ldy, P, float(eps), int(max_iter),
+                                   X.data_ptr(), R.data_ptr(), n_iter.data_ptr(),
+                                   idx_trace.data_ptr() if trace else None, c_trace.data_ptr() if trace else None, ldt,
+                                   base + off, workspace.numel() - off, _stream_ptr(stream)))
     return Recovered(X, R, n_iter, idx_trace, c_trace, workspace)
 
 

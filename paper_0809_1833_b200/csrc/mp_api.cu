@@ -135,6 +135,13 @@ static int64_t* option_slot(const char* name)
     if (!strcmp(name, "info_algo")) return &o.info_algo;
     if (!strcmp(name, "omp_algo")) return &o.omp_algo;
     if (!strcmp(name, "info_omp_algo")) return &o.info_omp_algo;
+    if (!strcmp(name, "many_cluster")) return &o.many_cluster;
+    if (!strcmp(name, "many_threads")) return &o.many_threads;
+    if (!strcmp(name, "many_stat")) return &o.many_stat;
+    if (!strcmp(name, "info_many_cluster")) return &o.info_many_cluster;
+    if (!strcmp(name, "info_many_stat")) return &o.info_many_stat;
+    if (!strcmp(name, "info_many_clusters")) return &o.info_many_clusters;
+    if (!strcmp(name, "info_many_threads")) return &o.info_many_threads;
     if (!strcmp(name, "info_tc_clusters")) return &o.info_tc_clusters;
     if (!strcmp(name, "info_tc_at")) return &o.info_tc_at;
     if (!strcmp(name, "info_tc_stages")) return &o.info_tc_stages;
@@ -205,8 +212,14 @@ mp_status mp_recover(const float* psi_t, int N, int M, int64_t ld,
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     const int64_t algo = options().algo;
     int64_t use = algo;
-    if (use < 1 || use > 3) use = persistent_ldg_supported(N, M) ? 3 : persistent_supported(N, M) ? 1 : 2;
+    if (use < 1 || use > 4)
+        use = many_single_stationary(N, M) ? 4 : persistent_ldg_supported(N, M) ? 3 : persistent_supported(N, M) ? 1 : 2;
     options().info_algo = use;
+    if (use == 4) {                                                 // one thread-block cluster, dictionary stationary in shared memory
+        if (!many_supported(N, M)) return fail(MP_ERR_UNSUPPORTED, "algo 4 (cluster kernel) needs N <= 2048 (got %d)", N);
+        ManyArgs m{psi_t, N, M, ld, 0, y, N, 1, eps, max_iter, x, r, n_iter, idx_trace, c_trace, max_iter};
+        return launch_recover_many(m, reinterpret_cast<unsigned int*>(ws.ctrl), s);
+    }
     if (use == 3) return launch_recover_persistent_ldg(a, ws, s);
     if (use == 1) return launch_recover_persistent(a, ws, s);
     return launch_recover_streamloop(a, ws, s);
@@ -279,6 +292,49 @@ size_t mp_correlate_batched_workspace_bytes(int N, int M, int B)
     const int Bw = B < 2 ? 2 : B;
     const size_t scratch_off = (mp_workspace_bytes(N, M, Bw) + 255) / 256 * 256;
     return scratch_off + sizeof(float) * ((size_t)Bw * M + (size_t)Bw * N) + sizeof(int) * (size_t)Bw + 512;
+}
+
+size_t mp_workspace_bytes_many(int N, int M, int P)
+{
+    if (N < 1 || M < 1 || P < 1) return 0;
+    return 256 + mp_workspace_bytes(N, M, 1);
+}
+
+mp_status mp_recover_many(const float* psi_t, int N, int M, int64_t ld, int64_t problem_stride,
+                          const float* Y, int64_t ldy, int P, float eps, int max_iter,
+                          float* X, float* R, int* n_iter,
+                          int* idx_trace, float* c_trace, int64_t ldt,
+                          void* workspace, size_t workspace_bytes, void* stream)
+{
+    mp_status st = check_dictionary(psi_t, N, M, ld);
+    if (st != MP_OK) return st;
+    if (P < 1) return fail(MP_ERR_INVALID_ARG, "need P >= 1 (got %d)", P);
+    if (problem_stride != 0 && (problem_stride < (int64_t)M * ld || (problem_stride & 3)))
+        return fail(MP_ERR_INVALID_ARG, "problem_stride must be 0 (one shared dictionary) or >= M*ld and a multiple of 4 floats");
+    if (!Y || !X || !R || !n_iter) return fail(MP_ERR_INVALID_ARG, "Y, X, R and n_iter must be non-null");
+    if (ldy < N) return fail(MP_ERR_INVALID_ARG, "need ldy >= N");
+    if (max_iter < 0) return fail(MP_ERR_INVALID_ARG, "max_iter must be >= 0 (got %d)", max_iter);
+    if (!(eps >= 0.0f)) return fail(MP_ERR_INVALID_ARG, "eps must be >= 0 and not NaN");
+    if ((idx_trace || c_trace) && ldt < max_iter) return fail(MP_ERR_INVALID_ARG, "need ldt >= max_iter");
+    const size_t need = mp_workspace_bytes_many(N, M, P);
+    if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 255u) || workspace_bytes < need)
+        return fail(MP_ERR_WORKSPACE, "workspace must be non-null, 256-byte aligned and >= %zu bytes (got %zu)", need, workspace_bytes);
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    if (many_supported(N, M)) {
+        ManyArgs a{psi_t, N, M, ld, problem_stride, Y, ldy, P, eps, max_iter, X, R, n_iter, idx_trace, c_trace, ldt};
+        return launch_recover_many(a, static_cast<unsigned int*>(workspace), s);
+    }
+    // long residuals (N > 2048): these are not "small" problems -- one grid-wide single-signal solve after another
+    char* ws1 = static_cast<char*>(workspace) + 256;
+    for (int q = 0; q < P; q++) {
+        st = mp_recover(psi_t + (int64_t)q * problem_stride, N, M, ld, Y + (int64_t)q * ldy, eps, max_iter,
+                        X + (int64_t)q * M, R + (int64_t)q * N, n_iter + q,
+                        idx_trace ? idx_trace + (int64_t)q * ldt : nullptr, c_trace ? c_trace + (int64_t)q * ldt : nullptr,
+                        ws1, workspace_bytes - 256, s);
+        if (st != MP_OK) return st;
+    }
+    options().info_many_cluster = 0;
+    return MP_OK;
 }
 
 // ---------------------------------------------------------------------------------------------------------

@@ -22,6 +22,8 @@ struct Options {
     int64_t algo = 0, warps = 0, slot_bytes = 0, depth = 0, grid = 0, chunk = 64;
     int64_t batched_algo = 0, batched_coop = 1;
     int64_t omp_algo = 0, info_omp_algo = 0;   // Orthogonal MP: 0 auto, 1 persistent kernel, 2 stream loop; and the one last used
+    int64_t many_cluster = 0, many_threads = 0, many_stat = 0;   // cluster-per-problem kernel: CTAs per problem (0 auto), threads per CTA (0 auto), 2 = never stationary
+    int64_t info_many_cluster = 0, info_many_stat = 0, info_many_clusters = 0, info_many_threads = 0;   // plan of its last launch
     int64_t info_algo = 0;             // kernel the last mp_recover call used (1, 2 or 3)
     int64_t info_tc_clusters = 0, info_tc_at = 0, info_tc_stages = 0;   // plan of the last batched tensor-core launch (read-only use)
 };
@@ -82,5 +84,15 @@ mp_status launch_recover_batched(const BatchedArgs& a, const Workspace& ws, cuda
 // tensor-core lock-step kernel (B <= 64 per launch); dbg_C (nullable, B x M) receives the correlations of iteration 0
 mp_status launch_recover_batched_tc(const BatchedArgs& a, const Workspace& ws, float* dbg_C, cudaStream_t stream);
 bool batched_tc_supported(int N, int M, int B);
+
+// P independent problems of one shape, one thread-block cluster per problem (mp_many.cu)
+struct ManyArgs {
+    const float* psi_t; int N, M; int64_t ld, pstride;
+    const float* Y; int64_t ldy; int P; float eps; int max_iter;
+    float* X; float* R; int* n_iter; int* idx_trace; float* c_trace; int64_t ldt;
+};
+bool many_supported(int N, int M);
+bool many_single_stationary(int N, int M);
+mp_status launch_recover_many(const ManyArgs& a, unsigned int* counter, cudaStream_t stream);
 
 }  // namespace mp

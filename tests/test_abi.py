@@ -88,3 +88,20 @@ def test_argument_errors_of_the_widened_entry_points():
     assert h(ok, 8, 8, 8, ok, 8, 65, ok, ok, 1 << 20, None) == 1                              # B > 64
     assert h(ok, 8, 8, 8, ok, 8, 2, ok, ok, 16, None) == 4
     assert lib.mp_correlate_batched_workspace_bytes(8, 8, 65) == 0
+
+
+def test_argument_errors_of_mp_recover_many():
+    from paper_0809_1833_b200.binding import lib
+    ok = C.c_void_p(4096)
+    f = lib.mp_recover_many
+    good = dict(psi=ok, N=8, M=8, ld=8, ps=64, Y=ok, ldy=8, P=2, eps=0.1, T=4, X=ok, R=ok, n=ok, it=None, ct=None, ldt=4, ws=ok, wsb=1 << 20)
+
+    def call(**kw):
+        a = dict(good, **kw)
+        return f(a["psi"], a["N"], a["M"], a["ld"], a["ps"], a["Y"], a["ldy"], a["P"], a["eps"], a["T"], a["X"], a["R"], a["n"],
+                 a["it"], a["ct"], a["ldt"], a["ws"], a["wsb"], None)
+    assert call(psi=None) == 1 and call(P=0) == 1 and call(ps=32) == 1 and call(ps=66) == 1        # stride < M*ld, stride % 4
+    assert call(ldy=4) == 1 and call(T=-1) == 1 and call(eps=-1.0) == 1 and call(Y=None) == 1
+    assert call(it=ok, ldt=2) == 1                                                                # ldt < max_iter
+    assert call(ws=None) == 4 and call(wsb=16) == 4
+    assert lib.mp_workspace_bytes_many(8, 8, 0) == 0 and lib.mp_workspace_bytes_many(8, 8, 3) >= 256

@@ -41,7 +41,8 @@ def run_single(mp, psi32, y32, eps, max_iter, algo=0, ld=None):
     return (res.x.cpu().numpy(), res.r.cpu().numpy(), t, res.idx_trace.cpu().numpy()[:t], res.c_trace.cpu().numpy()[:t])
 
 
-ALGOS = [1, 2, 3]      # 1 = TMA-staged persistent kernel, 2 = stream loop, 3 = register-streaming persistent kernel
+ALGOS = [1, 2, 3, 4]   # 1 = TMA-staged persistent kernel, 2 = stream loop, 3 = register-streaming persistent kernel,
+                       # 4 = one thread-block cluster (the mp_recover_many kernel with P = 1; N <= 2048)
 
 
 # ------------------------------------------------------------------------------------------ normalisation (a0)
@@ -107,6 +108,8 @@ RAGGED = [
 @pytest.mark.parametrize("algo", ALGOS)
 @pytest.mark.parametrize("N,M,K,ld", RAGGED)
 def test_ragged_shapes_full_grading(mp, N, M, K, ld, algo):
+    if algo == 4 and N > 2048:
+        pytest.skip("the cluster kernel holds the residual in registers: N <= 2048")
     cfg = problems.custom_config(N, M, K, eps=1e-4, max_iter=6 * K + 3)
     pb = problems.make_problem(cfg, seed=4)
     x, r, t, idx, cc = run_single(mp, pb.psi32, pb.Y[0], cfg.eps, cfg.max_iter, algo, ld)
