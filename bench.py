@@ -196,6 +196,9 @@ def main():
     ap.add_argument("--f64", action="store_true", help="double-precision path (mp_recover_f64) on the same workload shape")
     ap.add_argument("--omp", action="store_true", help="Orthogonal MP (mp_recover_omp) on the same workload")
     ap.add_argument("--signs", action="store_true", help="sign-packed Bernoulli dictionary (mp_recover_signs); Bernoulli configs only")
+    ap.add_argument("--phase", default=None, metavar="RHO,SIGMA[,TRIALS]",
+                    help="one cell of the paper's Fig. 1 phase diagram (P:92-106): M=1000, N=rho*M, K=sigma*M, TRIALS independent "
+                         "problems each with its own Bernoulli dictionary, eps=1e-7, T=N, solved by one mp_recover_many launch")
     ap.add_argument("--knob", action="append", default=[], metavar="NAME=VALUE", help="mp_set_int knob (profiling runs)")
     args = ap.parse_args()
     cfg = synth.config(args.config)
@@ -212,6 +215,8 @@ def main():
     for kv in args.knob:
         name, _, val = kv.partition("=")
         mp.mp_set_int(name, int(val))
+    if args.phase:
+        return run_phase(args, torch, mp)
     if args.f64:
         return run_f64(args, cfg, torch, mp)
     if args.omp:
@@ -531,6 +536,88 @@ def run_signs(args, cfg, torch, mp):
                      "peak_source": "%d SMs x 128 fp32 lanes x 1.965 GHz, one lane-op per dictionary entry (a test plus an add is two)" % sm,
                      "kernel": "mp_persistent_signs_kernel", "kernel_ms": solve_ms, "us_per_iteration": 1e3 * solve_ms / max(its, 1)},
         "cpu_baseline": None, "e2e": None}))
+
+
+def run_phase(args, torch, mp):
+    """One (sigma, rho) cell of the paper's Fig. 1 experiment (NEXT 4), 1 GPU: TRIALS independent problems, each with its own
+    Bernoulli dictionary (Eq. 13) and K nonzeros from U[-1, 1], eps = 1e-7, T = N.  One step = one
+    mp_recover_many launch over all trials.  The dictionaries in flight are L2-resident by plan, so the bound is L2 bandwidth."""
+    import oracle
+    parts = [float(v) for v in args.phase.split(",")]
+    rho, sigma = parts[0], parts[1]
+    P = int(parts[2]) if len(parts) > 2 else 400
+    M = 1000
+    N = max(4, int(round(rho * M / 4.0)) * 4)                  # ld % 4 == 0 at the boundary: N rounded to a multiple of 4
+    K = max(1, int(round(sigma * M)))
+    cfg = synth.Config("phase", N, M, K, "bernoulli", "uniform", 1e-7, N, 1)
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(0)
+    psi_h = torch.empty((P, M, N), dtype=torch.float32).pin_memory()
+    Y_h = torch.empty((P, N), dtype=torch.float32).pin_memory()
+    X_true = np.zeros((P, M))
+    for q in range(P):
+        d = synth.make_dictionary(cfg, 1000 + q)
+        x, S = synth.sparse_signal(M, K, 1000 + q, cfg.values)
+        psi_h[q] = torch.from_numpy(d); Y_h[q] = torch.from_numpy(synth.encode(d, x, S)); X_true[q] = x
+    psi_d, Y_d = psi_h.to(dev), Y_h.to(dev)
+    stream = torch.cuda.current_stream()
+    res = None
+    for _ in range(max(args.warmup, 1)):
+        res = mp.mp_recover_many(psi_d, Y_d, cfg.eps, cfg.max_iter, workspace=res.workspace if res else None)
+    clocks = ClockSampler(0); clocks.start()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0 = mp.mp_launch_count()
+    e0.record(stream)
+    for _ in range(args.steps):
+        res = mp.mp_recover_many(psi_d, Y_d, cfg.eps, cfg.max_iter, workspace=res.workspace)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    clk = clocks.stop()
+    launches = mp.mp_launch_count() - l0
+    ms = e0.elapsed_time(e1) / args.steps
+    its = int(res.n_iter.sum().item())
+    Xg = res.x.cpu().numpy().astype(np.float64)
+    err = [oracle.reconstruction_error_pct(Xg[q], X_true[q]) for q in range(P)]      # Eq. 14, outside the timed region
+    ach = its * 4.0 * N * M / (ms * 1e-3) / 1e9
+    l2_peak = 17500.0
+    out = {
+        "metric": METRIC, "value": its / (ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"phase-diagram cell rho={N / M:g}, sigma={K / M:g}: {P} trials, M={M}, N={N}, K={K}, own Bernoulli dictionary per trial, "
+                               f"U[-1,1] nonzeros, eps=1e-07, T=N", "iterations_per_step": its, "step": "one mp_recover_many launch over all trials",
+                   "l2": "by plan the dictionaries of the clusters in flight fit in L2; all trials together (%.0f MB) do not" % (P * 4.0 * N * M / 1e6),
+                   "parallelism": "1 GPU"},
+        "solves_per_s": P / (ms * 1e-3), "mean_error_pct_eq14": float(np.mean(err)), "mean_iterations": its / P,
+        "plan": {"threads": mp.mp_get_int("info_many_threads"), "cluster": mp.mp_get_int("info_many_cluster"),
+                 "stationary": mp.mp_get_int("info_many_stat"), "clusters_in_flight": mp.mp_get_int("info_many_clusters")},
+        "gpu_launches": int(launches), "clocks": clk,
+        "roofline": {"bound": "l2", "achieved": ach, "peak": l2_peak, "unit": "GB/s", "frac": ach / l2_peak, "traffic": None,
+                     "peak_source": "plain 128-bit loads of an L2-resident buffer on this pool's B200 (profiles/persistent_r01.md: 17-18 TB/s)",
+                     "kernel": "mp_many_kernel", "kernel_ms": ms, "algorithmic_bytes_per_launch": its * 4.0 * N * M},
+    }
+    if not args.no_cpu_baseline:
+        th = oracle.default_threads()
+        t0 = time.perf_counter(); n_ref = 0; q = 0
+        while q < P and time.perf_counter() - t0 < 10.0:
+            n_ref += oracle.mp(psi_h[q].numpy(), Y_h[q].numpy().astype(np.float64), float(np.float32(cfg.eps)), cfg.max_iter, th).n_iter; q += 1
+        dt = time.perf_counter() - t0
+        out["cpu_baseline"] = {"value": n_ref / dt, "unit": UNIT, "cores": th, "kind": "oracle",
+                               "sample": f"the first {q} trials of the cell, one after another (float64 C oracle, OpenMP over atoms, {th} threads)"}
+    if not args.no_e2e:
+        Xh = torch.empty((P, M), dtype=torch.float32).pin_memory(); nh = torch.empty(P, dtype=torch.int32).pin_memory()
+        t_best = None
+        for _ in range(2):
+            torch.cuda.synchronize(); t0 = time.perf_counter()
+            pd = psi_h.to(dev, non_blocking=True); yd = Y_h.to(dev, non_blocking=True)
+            r2 = mp.mp_recover_many(pd, yd, cfg.eps, cfg.max_iter, workspace=res.workspace)
+            Xh.copy_(r2.x, non_blocking=True); nh.copy_(r2.n_iter, non_blocking=True)
+            torch.cuda.synchronize(); dt = time.perf_counter() - t0
+            t_best = dt if t_best is None else min(t_best, dt)
+        out["e2e"] = {"value": int(nh.sum().item()) / t_best, "unit": UNIT, "h2d_bytes_per_step": int(psi_h.numel() * 4 + Y_h.numel() * 4),
+                      "d2h_bytes_per_step": int(Xh.numel() * 4 + nh.numel() * 4), "ms_per_step": t_best * 1e3,
+                      "note": "pinned host dictionaries and measurements -> device, mp_recover_many, x~ and n_iter -> pinned host, per step"}
+    print(json.dumps(out))
 
 
 def mp_kernel_name(mp):
