@@ -146,7 +146,7 @@ MP_API mp_status mp_recover_f64(const double* psi_t, int N, int M, int64_t ld,
 /* ---- Orthogonal Matching Pursuit (the paper's declared next target) -------------
  * MP's selection (Eq. 9, Eq. 16: fp32 dots of the fp32 rounding of r, lowest index on ties) followed by a least-squares
  * refit on the selected atoms, so that r = y - Psi_S x_S with x_S = argmin ||y - Psi_S z||_2 after every step.  The refit is
- * a float64 QR factorisation grown by one column per iteration (Gram-Schmidt applied twice); x~ is obtained once, at the
+ * a float64 QR factorisation grown by one column per iteration (Gram-Schmidt, a second pass whenever the first removed more than half of the atom); x~ is obtained once, at the
  * end, by back substitution.  Stop rule as MP; at most min(max_iter, N) atoms are taken; an atom that lies in the
  * span of the selected ones ends the run.  Same layouts as mp_recover; idx_trace (nullable) receives the atoms in order.
  * Runs as one persistent cooperative kernel when the orthonormal basis, sliced by components over the CTAs, fits in shared
