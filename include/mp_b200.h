@@ -21,7 +21,7 @@
  *     n = 0..N-1, ld >= N and ld % 4 == 0.  (= Psi^T row-major = Psi column-major; each atom is
  *     contiguous so the reduction over n is coalesced.)  Elements psi_t[m*ld + n], N <= n < ld, may
  *     be read by the library but never influence a result.  The paper's own layout (Psi row-major,
- *     A2 P:360) is NOT accepted.
+ *     A2 P:360) is NOT accepted by the solvers; mp_transpose_rowmajor converts it once.
  *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Calls are
  *     asynchronous on `stream`: they validate arguments on the host, enqueue work and return; they
  *     never synchronise the host (exception: the stream-loop fallback algorithm, see mp_set_int).
@@ -68,6 +68,12 @@ MP_API size_t mp_workspace_bytes(int N, int M, int B);
  * scaling.  The paper assumes Eq. 4 and never executes it (its Bernoulli atoms are unit by
  * construction, Eq. 13). */
 MP_API mp_status mp_normalize_columns(float* psi_t, int N, int M, int64_t ld, float* norms_out, void* stream);
+
+/* Ingestion of the paper's own layout.  The listings hold Psi ROW-MAJOR, psi[n*ldr + m] (A2 P:360,
+ * P:424; ldr >= M, any alignment), which makes every atom a stride-M gather (the axpy column of A2 P:470); this copies it once
+ * into the atom-major psi_t[m*ld + n] every other entry point takes (ld >= N, ld % 4 == 0, 16-byte aligned).  Out of place
+ * (overlapping buffers are refused), bit-exact, HBM-bound (8NM bytes); elements psi_t[m*ld + n], n >= N, are not written. */
+MP_API mp_status mp_transpose_rowmajor(const float* psi, int N, int M, int64_t ldr, float* psi_t, int64_t ld, void* stream);
 
 /* The MP loop above for one signal.
  *   psi_t      in   dictionary, ASSUMED column-normalised (not checked; the update uses <r,psi_i> as is)

@@ -15,7 +15,7 @@ import numpy as np
 from . import build as _build
 
 __all__ = ["normalize_columns", "correlate", "argmax_abs", "nrm2", "mp", "mp_replay",
-           "mp_batched", "omp", "OMPResult", "encode_sparse", "reconstruction_error_pct", "MPResult", "ReplayResult", "default_threads"]
+           "mp_batched", "omp", "OMPResult", "encode_sparse", "atom_major_from_rowmajor", "reconstruction_error_pct", "MPResult", "ReplayResult", "default_threads"]
 
 _lib = C.CDLL(_build.build())
 
@@ -245,3 +245,14 @@ def encode_sparse(psi_t, idx, val) -> np.ndarray:
 def reconstruction_error_pct(x_hat, x) -> float:
     x_hat, x = _f64(x_hat), _f64(x)
     return _lib.oracle_reconstruction_error_pct(_ptr(x_hat), _ptr(x), x.size)
+
+
+def atom_major_from_rowmajor(psi) -> np.ndarray:
+    """The paper's listings store Psi row-major, psi[n*M + m] (A2 P:360: `h_Psi[n*M + m]`); every routine here takes the
+    atom-major psi_t[m, n] = Psi[n, m].  The definition written out, element by element (no arithmetic)."""
+    psi = np.asarray(psi)
+    N, M = psi.shape
+    out = np.empty((M, N), dtype=psi.dtype)
+    for n in range(N):
+        out[:, n] = psi[n, :]
+    return out

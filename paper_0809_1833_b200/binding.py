@@ -72,6 +72,8 @@ lib.mp_pack_signs.restype = _i
 lib.mp_pack_signs.argtypes = [_vp, _i, _i, _i64, _vp, _i64, _vp, _vp, _vp]
 lib.mp_recover_signs.restype = _i
 lib.mp_recover_signs.argtypes = [_vp, _i, _i, _i64, _f, _vp, _f, _i, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]
+lib.mp_transpose_rowmajor.restype = _i
+lib.mp_transpose_rowmajor.argtypes = [_vp, _i, _i, _i64, _vp, _i64, _vp]
 lib.mp_workspace_bytes_many.restype = _sz
 lib.mp_workspace_bytes_many.argtypes = [_i, _i, _i]
 lib.mp_recover_many.restype = _i
@@ -152,6 +154,23 @@ def mp_normalize_columns(psi_t: torch.Tensor, norms_out: torch.Tensor | None = N
     n = _dev(norms_out, torch.float32, "norms_out") if norms_out is not None else None
     with torch.cuda.device(psi_t.device):
         _check(lib.mp_normalize_columns(p, N, M, ld, n, _stream_ptr(stream)))
+
+
+def mp_transpose_rowmajor(psi: torch.Tensor, psi_t: torch.Tensor | None = None, stream=None) -> torch.Tensor:
+    """The paper's row-major Psi[N, M] (A2 P:360) -> the atom-major psi_t[M, N] the solvers take (row stride padded to 4)."""
+    if not (psi.is_cuda and psi.dtype == torch.float32 and psi.dim() == 2 and (psi.shape[1] == 1 or psi.stride(1) == 1)):
+        raise TypeError("psi must be a CUDA float32 [N, M] tensor with unit stride along M (row-major Psi)")
+    N, M = psi.shape
+    ldr = psi.stride(0) if N > 1 else max(psi.stride(0), M)
+    if psi_t is None:
+        ld = (N + 3) // 4 * 4
+        psi_t = torch.zeros((M, ld), dtype=torch.float32, device=psi.device)[:, :N]
+    p, N2, M2, ld = _dict_args(psi_t)
+    if (N2, M2) != (N, M):
+        raise ValueError("psi_t must be [M, N]")
+    with torch.cuda.device(psi.device):
+        _check(lib.mp_transpose_rowmajor(psi.data_ptr(), N, M, ldr, p, ld, _stream_ptr(stream)))
+    return psi_t
 
 
 @dataclasses.dataclass

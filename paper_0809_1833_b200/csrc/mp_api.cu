@@ -172,6 +172,19 @@ mp_status mp_normalize_columns(float* psi_t, int N, int M, int64_t ld, float* no
     return launch_normalize(psi_t, N, M, ld, norms_out, static_cast<cudaStream_t>(stream));
 }
 
+mp_status mp_transpose_rowmajor(const float* psi, int N, int M, int64_t ldr, float* psi_t, int64_t ld, void* stream)
+{
+    if (!psi) return fail(MP_ERR_INVALID_ARG, "psi is null");
+    if (ldr < M) return fail(MP_ERR_INVALID_ARG, "need ldr >= M (got ldr=%lld, M=%d)", (long long)ldr, M);
+    mp_status st = check_dictionary(psi_t, N, M, ld);
+    if (st != MP_OK) return st;
+    const char* a = reinterpret_cast<const char*>(psi);
+    const char* b = reinterpret_cast<const char*>(psi_t);
+    if (a < b + sizeof(float) * (size_t)M * ld && b < a + sizeof(float) * (size_t)N * ldr)
+        return fail(MP_ERR_INVALID_ARG, "psi and psi_t overlap: the transpose is out of place");
+    return launch_transpose_rowmajor(psi, N, M, ldr, psi_t, ld, static_cast<cudaStream_t>(stream));
+}
+
 mp_status mp_encode_sparse(const float* psi_t, int N, int M, int64_t ld, const int* idx, const float* val, int K,
                            float* y, void* stream)
 {

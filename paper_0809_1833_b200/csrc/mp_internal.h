@@ -54,6 +54,8 @@ static inline int round_up(int v, int m) { return (v + m - 1) / m * m; }
 // ---- launchers (each enqueues on `stream`, returns MP_OK or an error) ---------------------------------------
 mp_status launch_normalize(float* psi_t, int N, int M, int64_t ld, float* norms_out, cudaStream_t stream);
 
+mp_status launch_transpose_rowmajor(const float* psi, int N, int M, int64_t ldr, float* psi_t, int64_t ld, cudaStream_t stream);
+
 mp_status launch_encode_sparse(const float* psi_t, int N, int M, int64_t ld, const int* idx, const float* val, int K,
                                float* y, cudaStream_t stream);
 mp_status launch_reconstruction_error(const float* x_hat, const float* x, int M, double* out, cudaStream_t stream);

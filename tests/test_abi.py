@@ -105,3 +105,13 @@ def test_argument_errors_of_mp_recover_many():
     assert call(it=ok, ldt=2) == 1                                                                # ldt < max_iter
     assert call(ws=None) == 4 and call(wsb=16) == 4
     assert lib.mp_workspace_bytes_many(8, 8, 0) == 0 and lib.mp_workspace_bytes_many(8, 8, 3) >= 256
+
+
+def test_argument_errors_of_mp_transpose_rowmajor():
+    from paper_0809_1833_b200.binding import lib
+    ok, ok2 = C.c_void_p(4096), C.c_void_p(1 << 30)
+    f = lib.mp_transpose_rowmajor
+    assert f(None, 8, 8, 8, ok2, 8, None) == 1 and f(ok, 8, 8, 8, None, 8, None) == 1
+    assert f(ok, 8, 8, 7, ok2, 8, None) == 1                                   # ldr < M
+    assert f(ok, 8, 8, 8, ok2, 6, None) == 1                                   # ld < N / ld % 4
+    assert f(ok, 8, 8, 8, C.c_void_p(4096 + 64), 8, None) == 1                 # overlapping buffers

@@ -513,3 +513,24 @@ def test_omp_two_atom_closed_form_and_edge_cases():
     assert oracle.omp(psi3, rng.standard_normal(6), 0.0, 100).n_iter <= 6
     dup = oracle.omp(psi3, rng.standard_normal(6), 0.0, 0, idx_force=[3, 5, 3])
     assert dup.status == 2 and dup.n_iter == 2
+
+
+def test_rowmajor_ingestion_is_the_index_swap_and_keeps_the_method():
+    """atom_major_from_rowmajor: psi_t[m, n] = Psi[n, m] checked index by index, and MP on the converted dictionary equals a
+    numpy gemv/argmax/axpy loop run directly on the paper's row-major array (A2 P:464-471 in that layout)."""
+    rng = np.random.default_rng(21)
+    N, M = 7, 11
+    psi = rng.standard_normal((N, M))
+    psi /= np.linalg.norm(psi, axis=0, keepdims=True)
+    pt = oracle.atom_major_from_rowmajor(psi)
+    assert pt.shape == (M, N) and all(pt[m, n] == psi[n, m] for m in range(M) for n in range(N))
+    x = np.zeros(M); x[[2, 9]] = [1.5, -0.7]
+    y = psi @ x
+    res = oracle.mp(pt, y, 0.0, 6)
+    r = y.copy(); xs = np.zeros(M)
+    for t in range(6):
+        c = psi.T @ r                                   # gemv on the row-major array
+        i = int(np.argmax(np.abs(c)))                   # first occurrence = lowest index
+        xs[i] += c[i]; r = r - c[i] * psi[:, i]         # axpy with the stride-M column
+        assert res.idx[t] == i
+    assert np.allclose(res.x, xs, atol=1e-14) and np.allclose(res.r, r, atol=1e-14)
