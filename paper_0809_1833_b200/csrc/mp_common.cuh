@@ -139,4 +139,41 @@ __device__ __forceinline__ void red_add_f64(double* p, double v)
     asm volatile("red.relaxed.gpu.global.add.f64 [%0], %1;" ::"l"(p), "d"(v) : "memory");
 }
 
+// ------------------------------------------------------------------------------------------------
+// L2 residency control.  A dictionary larger than L2, streamed cyclically, gets no reuse at all (ncu: DRAM traffic = 4NM
+// per iteration, L2 hit rate 0.2 %).  Loading a FIXED subset of the rows with the evict_last priority and the rest with
+// evict_first keeps that subset in L2 across iterations, so only the rest comes from HBM every iteration.  Measured on
+// B200 (profiles/persistent_r01.md): ~64-72 MB stay resident (more thrashes), CFG3 40.5 -> 33.2 us per iteration.
+__device__ __forceinline__ uint64_t l2_policy_evict_last()
+{
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ uint64_t l2_policy_evict_first()
+{
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ float4 ldg_cg4_hint(const float4* p, uint64_t policy)
+{
+    float4 v;
+    asm volatile("ld.global.cg.L2::cache_hint.v4.f32 {%0, %1, %2, %3}, [%4], %5;"
+                 : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p), "l"(policy));
+    return v;
+}
+
+__device__ __forceinline__ double2 ldg_cg_d2_hint(const double2* p, uint64_t policy)
+{
+    double2 v;
+    asm volatile("ld.global.cg.L2::cache_hint.v2.f64 {%0, %1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(p), "l"(policy));
+    return v;
+}
+// group g of n_groups is one of the rg resident ones (spread evenly: L2 hits and HBM misses interleave in time)
+__device__ __forceinline__ bool l2_group_is_resident(int g, int rg, int n_groups)
+{
+    return ((g + 1) * rg) / n_groups != (g * rg) / n_groups;
+}
+
 }  // namespace mp

@@ -36,6 +36,7 @@ struct F64Params {
     int N, M, Npad, Nr;         // Npad = N rounded up to 2, Nr = N rounded up to 128
     double eps;
     int max_iter;
+    int resident_groups;        // groups of A atoms per CTA loaded L2::evict_last (mp_common.cuh), 0 = no hints
 };
 
 __device__ __forceinline__ double2 ldg_cg_d2(const double2* p)
@@ -103,9 +104,25 @@ mp_persistent_f64_kernel(const F64Params p)
 
     const double2* r2 = reinterpret_cast<const double2*>(rres);
     double2 v[A][UC];
+    const uint64_t pol_last = l2_policy_evict_last(), pol_first = l2_policy_evict_first();
     auto load_item = [&](int item) {
         const int g = item / n_chunks, ch = item - g * n_chunks;
         const int jb = ch * 32 * UC + lane;
+        if (A <= 4 && p.resident_groups > 0) {                                  // dictionary larger than L2: residency hints (long rows only:
+                                                                                // the short-row variants have no registers to spare)
+            const uint64_t pol = l2_group_is_resident(g, p.resident_groups, n_groups) ? pol_last : pol_first;
+#pragma unroll
+            for (int a = 0; a < A; a++) {
+                const int rel = g * A + a < n_atoms ? g * A + a : n_atoms - 1;
+                const double2* row = reinterpret_cast<const double2*>(p.psi_t + (int64_t)(a0 + rel) * p.ld);
+#pragma unroll
+                for (int u = 0; u < UC; u++) {
+                    const int j = jb + 32 * u;
+                    v[a][u] = j < n2 ? ldg_cg_d2_hint(row + j, pol) : make_double2(0.0, 0.0);
+                }
+            }
+            return;
+        }
 #pragma unroll
         for (int a = 0; a < A; a++) {
             const int rel = g * A + a < n_atoms ? g * A + a : n_atoms - 1;      // a short last group re-reads its last atom
@@ -358,6 +375,7 @@ MP_API mp_status mp_recover_f64(const double* psi_t, int N, int M, int64_t ld,
     p.slots = reinterpret_cast<Cand*>(base + 256 + (sizeof(double) * (size_t)M + 255) / 256 * 256);
     p.ld = ld; p.N = N; p.M = M; p.Npad = round_up(N, 2); p.Nr = round_up(N, 128);
     p.eps = eps; p.max_iter = max_iter;
+    p.resident_groups = l2_resident_groups(8.0 * (double)ld * M, plan.grid, 8.0 * (double)ld * plan.A);
     if (plan.A == 16) return launch_f64<16, 1>(p, plan, di.device, s);
     if (plan.A == 8) return launch_f64<8, 2>(p, plan, di.device, s);
     if (plan.A == 4) return launch_f64<4, 4>(p, plan, di.device, s);

@@ -51,6 +51,14 @@ struct Workspace {
 };
 size_t workspace_layout(int N, int M, int B, void* base, Workspace* ws);
 static inline int round_up(int v, int m) { return (v + m - 1) / m * m; }
+// L2 residency (mp_common.cuh): groups of rows per CTA to load with evict_last.  Only for dictionaries that do not fit in L2
+// anyway (> 72 MB); knob "l2_resident_mb": 0 = auto (68 MB, measured optimum on B200), 1 = off, else the MB to keep.
+static inline int l2_resident_groups(double dict_bytes, int grid, double group_bytes)
+{
+    const double target = options().l2_resident_mb == 0 ? 68e6 : options().l2_resident_mb == 1 ? 0.0 : 1e6 * (double)options().l2_resident_mb;
+    if (!(dict_bytes > 72e6) || !(target > 0.0) || grid < 1) return 0;
+    return (int)(target / grid / group_bytes);
+}
 
 // ---- launchers (each enqueues on `stream`, returns MP_OK or an error) ---------------------------------------
 mp_status launch_normalize(float* psi_t, int N, int M, int64_t ld, float* norms_out, cudaStream_t stream);

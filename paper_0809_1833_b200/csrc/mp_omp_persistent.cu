@@ -31,6 +31,7 @@ struct OmpPParams {
     int SLp;                    // padded (odd) pitch of a basis-vector slice in shared memory
     int atoms_max;
     float eps;
+    int resident_groups;        // groups of A atoms per CTA loaded L2::evict_last (mp_common.cuh), 0 = no hints
 };
 
 __device__ __forceinline__ float4 omp_ldg_cg4(const float4* p)
@@ -103,9 +104,25 @@ mp_omp_persistent_kernel(const OmpPParams p)
 
     const float4* r4 = reinterpret_cast<const float4*>(r32);
     float4 v[A][UC];
+    const uint64_t pol_last = l2_policy_evict_last(), pol_first = l2_policy_evict_first();
     auto load_item = [&](int item) {
         const int g = item / n_chunks, ch = item - g * n_chunks;
         const int jb = ch * 32 * UC + lane;
+        if (A <= 4 && p.resident_groups > 0) {                                  // dictionary larger than L2: residency hints (long rows only:
+                                                                                // the short-row variants have no registers to spare)
+            const uint64_t pol = l2_group_is_resident(g, p.resident_groups, n_groups) ? pol_last : pol_first;
+#pragma unroll
+            for (int a = 0; a < A; a++) {
+                const int rel = g * A + a < n_atoms ? g * A + a : n_atoms - 1;
+                const float4* row = reinterpret_cast<const float4*>(p.psi_t + (int64_t)(a0 + rel) * p.ld);
+#pragma unroll
+                for (int u = 0; u < UC; u++) {
+                    const int j = jb + 32 * u;
+                    v[a][u] = j < n4 ? ldg_cg4_hint(row + j, pol) : make_float4(0.f, 0.f, 0.f, 0.f);
+                }
+            }
+            return;
+        }
 #pragma unroll
         for (int a = 0; a < A; a++) {
             const int rel = g * A + a < n_atoms ? g * A + a : n_atoms - 1;
@@ -386,6 +403,7 @@ mp_status launch_omp_persistent(const OmpArgs& a, const OmpWs& ws, cudaStream_t 
     p.psi_t = a.psi_t; p.y = a.y; p.idx_trace = a.idx_trace; p.ws = ws; p.ld = a.ld;
     p.N = a.N; p.M = a.M; p.Npad = round_up(a.N, 4); p.Nr = round_up(a.N, 128); p.T = a.T; p.Tld = round_up(a.T, 32);
     p.SLp = plan.SLp; p.atoms_max = plan.atoms_max; p.eps = a.eps;
+    p.resident_groups = l2_resident_groups(4.0 * (double)a.ld * a.M, plan.grid, 4.0 * (double)a.ld * plan.A);
     if (plan.A == 16) return launch_omp_p<16, 1>(p, plan, di.device, stream);
     if (plan.A == 8) return launch_omp_p<8, 2>(p, plan, di.device, stream);
     if (plan.A == 4) return launch_omp_p<4, 4>(p, plan, di.device, stream);

@@ -40,30 +40,6 @@ struct LdgParams {
     int resident_groups;        // groups of A atoms per CTA loaded with L2::evict_last (0 = no residency hints)
 };
 
-// L2 residency control.  A dictionary larger than L2, streamed cyclically, gets no reuse at all (ncu: DRAM traffic = 4NM
-// per iteration, L2 hit rate 0.2 %).  Loading a FIXED subset of the rows with the evict_last priority and the rest with
-// evict_first keeps that subset in L2 across iterations, so only the rest comes from HBM every iteration.  Measured on
-// B200 (profiles/persistent_r01.md): ~64-72 MB stay resident (more thrashes), CFG3 40.5 -> 33.2 us per iteration.
-__device__ __forceinline__ uint64_t l2_policy_evict_last()
-{
-    uint64_t p;
-    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
-    return p;
-}
-__device__ __forceinline__ uint64_t l2_policy_evict_first()
-{
-    uint64_t p;
-    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
-    return p;
-}
-__device__ __forceinline__ float4 ldg_cg4_hint(const float4* p, uint64_t policy)
-{
-    float4 v;
-    asm volatile("ld.global.cg.L2::cache_hint.v4.f32 {%0, %1, %2, %3}, [%4], %5;"
-                 : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p), "l"(policy));
-    return v;
-}
-
 __device__ __forceinline__ float4 ldg_cg4(const float4* p)
 {
     float4 v;
@@ -120,11 +96,11 @@ mp_persistent_ldg_kernel(const LdgParams p)
     auto load_item = [&](int item) {
         const int g = item / n_chunks, ch = item - g * n_chunks;
         const int jb = ch * 32 * UC + lane;
-        if (p.resident_groups > 0) {                                            // dictionary larger than L2: residency hints
+        if (A <= 4 && p.resident_groups > 0) {                                  // dictionary larger than L2: residency hints (long rows only:
+                                                                                // the short-row variants have no registers to spare)
             // The resident groups are spread evenly over the CTA's share (Bresenham), so that L2 hits and HBM misses
             // interleave in time: with the resident rows first, HBM idled while every CTA read them (35.4 -> 33.3 us).
-            const int rg = p.resident_groups;
-            const uint64_t pol = ((g + 1) * rg) / n_groups != (g * rg) / n_groups ? pol_last : pol_first;
+            const uint64_t pol = l2_group_is_resident(g, p.resident_groups, n_groups) ? pol_last : pol_first;
 #pragma unroll
             for (int a = 0; a < A; a++) {
                 const int rel = g * A + a < n_atoms ? g * A + a : n_atoms - 1;
@@ -351,13 +327,7 @@ mp_status launch_recover_persistent_ldg(const RecoverArgs& a, const Workspace& w
     p.N = a.N; p.M = a.M; p.Npad = round_up(a.N, 4); p.Nr = round_up(a.N, 128);
     p.eps = a.eps; p.max_iter = a.max_iter;
     // L2 residency: only for dictionaries that do not fit in L2 anyway.  Knob "l2_resident_mb": 0 = auto (68 MB), 1 = off.
-    p.resident_groups = 0;
-    {
-        const double bytes = 4.0 * (double)a.ld * a.M;
-        const double target = options().l2_resident_mb == 0 ? 68e6 : options().l2_resident_mb == 1 ? 0.0 : 1e6 * (double)options().l2_resident_mb;
-        if (bytes > 72e6 && target > 0.0)
-            p.resident_groups = (int)(target / plan.grid / (4.0 * (double)a.ld * plan.A));
-    }
+    p.resident_groups = l2_resident_groups(4.0 * (double)a.ld * a.M, plan.grid, 4.0 * (double)a.ld * plan.A);
     if (plan.A == 16) return launch_ldg<16, 1>(p, plan, di.device, stream);
     if (plan.A == 8) return launch_ldg<8, 2>(p, plan, di.device, stream);
     if (plan.A == 4) return launch_ldg<4, 4>(p, plan, di.device, stream);
