@@ -217,8 +217,10 @@ MP_API const char* mp_last_error(void);
  *   "slot_bytes"    bytes of one shared-memory stage (0 = auto);   "depth"  stages per warp (0 = auto)
  *   "grid"          CTAs of the persistent kernel (0 = auto = one per SM)
  *   "chunk"         iterations enqueued between stop-flag polls of algo 2 (default 64)
- *   "batched_algo"  0 = auto (default): lock-step tensor-core kernel in groups of <= 64 signals when the shape fits,
- *                   1 = tensor-core kernel or MP_ERR_UNSUPPORTED, 2 = one single-signal solve after another
+ *   "batched_algo"  0 = auto (default): lock-step tensor-core kernel in groups of <= 64 signals when the shape fits and the
+ *                   dictionary is larger than 1.5 MB, else one thread-block cluster per signal (N <= 2048), else sequential;
+ *                   1 = tensor-core kernel or MP_ERR_UNSUPPORTED, 2 = one single-signal solve after another,
+ *                   3 = one cluster per signal (the mp_recover_many kernel on the shared dictionary) or MP_ERR_UNSUPPORTED
  *   "batched_coop"  1 (default) = launch the batched kernel with the cooperative attribute (co-residency checked by
  *                   the driver), 0 = plain cluster launch of a grid sized from cudaOccupancyMaxActiveClusters */
 MP_API mp_status mp_set_int(const char* name, int64_t value);

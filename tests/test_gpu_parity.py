@@ -250,7 +250,8 @@ def test_cfg3_full_size_sampled_grading(mp):
 
 
 # ------------------------------------------------------------------------------------------ batched (a9)
-BATCHED_ALGOS = [1, 2]        # 1 = lock-step tensor-core kernel (split-TF32 tcgen05), 2 = sequential single-signal solves
+BATCHED_ALGOS = [1, 2, 3]     # 1 = lock-step tensor-core kernel (split-TF32 tcgen05), 2 = sequential single-signal solves,
+                              # 3 = one thread-block cluster per signal on the shared dictionary
 
 
 @pytest.mark.parametrize("B,N,M", [(64, 2048, 8192), (7, 250, 333), (64, 128, 512), (1, 4096, 2048), (33, 1000, 9000)])
