@@ -571,15 +571,24 @@ def run_phase(args, torch, mp):
     psi_d, Y_d = psi_h.to(dev), Y_h.to(dev)
     stream = torch.cuda.current_stream()
     res = None
+    signs = bool(args.signs)
+
+    def step(ws):
+        if signs:                  # the same cell from one sign bit per entry: pack the stacked dictionaries, one CTA per problem
+            bits, scale, n_bad = mp.mp_pack_signs(psi_d.view(P * M, N))
+            assert n_bad == 0
+            return mp.mp_recover_signs_many(bits.view(P, M, -1), N, scale, Y_d, cfg.eps, cfg.max_iter, workspace=ws)
+        return mp.mp_recover_many(psi_d, Y_d, cfg.eps, cfg.max_iter, workspace=ws)
+
     for _ in range(max(args.warmup, 1)):
-        res = mp.mp_recover_many(psi_d, Y_d, cfg.eps, cfg.max_iter, workspace=res.workspace if res else None)
+        res = step(res.workspace if res else None)
     clocks = ClockSampler(0); clocks.start()
     torch.cuda.synchronize()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     l0 = mp.mp_launch_count()
     e0.record(stream)
     for _ in range(args.steps):
-        res = mp.mp_recover_many(psi_d, Y_d, cfg.eps, cfg.max_iter, workspace=res.workspace)
+        res = step(res.workspace)
     e1.record(stream)
     torch.cuda.synchronize()
     clk = clocks.stop()
@@ -605,6 +614,17 @@ def run_phase(args, torch, mp):
                      "peak_source": "plain 128-bit loads of an L2-resident buffer on this pool's B200 (profiles/persistent_r01.md: 17-18 TB/s)",
                      "kernel": "mp_many_kernel", "kernel_ms": ms, "algorithmic_bytes_per_launch": its * 4.0 * N * M},
     }
+    if signs:
+        sm = torch.cuda.get_device_properties(0).multi_processor_count
+        peak = sm * 128 * 1.965e9 / 1e12
+        ops = its * float(N) * M / 4.0 / (ms * 1e-3) / 1e12                    # one table lookup + add per four entries
+        out["config"]["workload"] += "; dictionaries as 1 sign bit per entry, one CTA per problem, bits stationary in shared memory"
+        out["config"]["step"] = "mp_pack_signs of the stacked dictionaries + one mp_recover_signs_many launch over all trials"
+        out["plan"] = None
+        out["roofline"] = {"bound": "alu", "achieved": ops, "peak": peak, "unit": "T lookup-adds/s", "frac": ops / peak, "traffic": None,
+                           "peak_source": "%d SMs x 128 fp32 lanes x 1.965 GHz; the lookup scheme needs one add per four dictionary entries "
+                                          "(plus a shift, a mask and a shared-memory load)" % sm,
+                           "kernel": "mp_many_signs_kernel", "kernel_ms": ms}
     if not args.no_cpu_baseline:
         th = oracle.default_threads()
         t0 = time.perf_counter(); n_ref = 0; q = 0
@@ -613,7 +633,7 @@ def run_phase(args, torch, mp):
         dt = time.perf_counter() - t0
         out["cpu_baseline"] = {"value": n_ref / dt, "unit": UNIT, "cores": th, "kind": "oracle",
                                "sample": f"the first {q} trials of the cell, one after another (float64 C oracle, OpenMP over atoms, {th} threads)"}
-    if not args.no_e2e:
+    if not args.no_e2e and not signs:
         Xh = torch.empty((P, M), dtype=torch.float32).pin_memory(); nh = torch.empty(P, dtype=torch.int32).pin_memory()
         t_best = None
         for _ in range(2):

@@ -180,6 +180,21 @@ MP_API mp_status mp_recover_signs(const uint32_t* bits, int N, int M, int64_t ld
                            float* x, float* r, int* n_iter, int* idx_trace, float* c_trace,
                            void* workspace, size_t workspace_bytes, void* stream);
 
+/* mp_recover_signs_many: P independent problems, each with its OWN sign-packed Bernoulli dictionary -- the paper's Fig. 1
+ * experiment in the paper's own representation.  bits: problem q's words start at bits + q*problem_stride (uint32
+ * words; [M][ldw] as mp_pack_signs writes them -- packing the P dictionaries stacked as one [P*M, N] dictionary gives exactly
+ * this with problem_stride = M*ldw; 0 = one shared dictionary).  Y P x N (row stride ldy >= N), X P x M, R P x N, n_iter P ints,
+ * traces nullable [q*ldt + t], ldt >= max_iter.  One CTA owns a problem: its N*M/8 bytes of bits stay in that SM's shared memory
+ * for the whole solve, and the correlations come from a per-iteration table of the 16 signed sums of every four residual values
+ * (one lookup per four entries).  Contract as mp_recover_signs (fp32 sums of the fp32 rounding of a float64 residual, lowest
+ * index on ties).  MP_ERR_UNSUPPORTED if bits + table do not fit in one SM's shared memory (N*M/8 + 28 N + 8 M > ~227 KB).
+ * Workspace: mp_workspace_bytes_signs_many(N, M, P) (256 bytes). */
+MP_API size_t mp_workspace_bytes_signs_many(int N, int M, int P);
+MP_API mp_status mp_recover_signs_many(const uint32_t* bits, int N, int M, int64_t ldw, int64_t problem_stride, float scale,
+                                const float* Y, int64_t ldy, int P, float eps, int max_iter,
+                                float* X, float* R, int* n_iter, int* idx_trace, float* c_trace, int64_t ldt,
+                                void* workspace, size_t workspace_bytes, void* stream);
+
 /* ---- many independent small problems (the paper's Fig. 1 experiment) -----------------
  * P problems of one shape (N, M), each with its OWN dictionary and measurement vector -- the (sigma, rho) phase diagram is
  * 100 trials per cell at M = 1000 with a fresh Bernoulli dictionary per trial -- solved by one launch:

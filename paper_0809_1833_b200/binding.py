@@ -78,6 +78,10 @@ lib.mp_workspace_bytes_many.restype = _sz
 lib.mp_workspace_bytes_many.argtypes = [_i, _i, _i]
 lib.mp_recover_many.restype = _i
 lib.mp_recover_many.argtypes = [_vp, _i, _i, _i64, _i64, _vp, _i64, _i, _f, _i, _vp, _vp, _vp, _vp, _vp, _i64, _vp, _sz, _vp]
+lib.mp_workspace_bytes_signs_many.restype = _sz
+lib.mp_workspace_bytes_signs_many.argtypes = [_i, _i, _i]
+lib.mp_recover_signs_many.restype = _i
+lib.mp_recover_signs_many.argtypes = [_vp, _i, _i, _i64, _i64, _f, _vp, _i64, _i, _f, _i, _vp, _vp, _vp, _vp, _vp, _i64, _vp, _sz, _vp]
 lib.mp_last_error.restype = C.c_char_p
 lib.mp_last_error.argtypes = []
 lib.mp_set_int.restype = _i
@@ -417,6 +421,40 @@ def mp_recover_signs(bits: torch.Tensor, N: int, scale: float, y: torch.Tensor, 
                                     idx_trace.data_ptr() if trace else None, c_trace.data_ptr() if trace else None,
                                     wp, wb, _stream_ptr(stream)))
     return Recovered(x, r, n_iter, idx_trace, c_trace, workspace)
+
+
+def mp_recover_signs_many(bits: torch.Tensor, N: int, scale: float, Y: torch.Tensor, eps: float, max_iter: int, *,
+                          trace: bool = False, workspace=None, stream=None) -> Recovered:
+    """P independent problems on sign-packed Bernoulli dictionaries (the paper's Fig. 1 workload in its own representation):
+    bits int32[P, M, ldw] (mp_pack_signs of the [P*M, N] stack, viewed per problem; [M, ldw] = one shared dictionary),
+    Y[P, N] -> X[P, M], R[P, N], n_iter[P] (+ traces); one CTA per problem, the bits stationary in its shared memory."""
+    if not (bits.is_cuda and bits.dtype == torch.int32 and bits.dim() in (2, 3) and bits.is_contiguous()):
+        raise TypeError("bits must be a contiguous CUDA int32 [P, M, ldw] (or [M, ldw]) tensor")
+    M, ldw = bits.shape[-2:]
+    dev = bits.device
+    if not (Y.is_cuda and Y.dtype == torch.float32 and Y.dim() == 2 and Y.shape[1] == N and (N == 1 or Y.stride(1) == 1)):
+        raise TypeError("Y must be a CUDA float32 [P, N] tensor with unit stride along N")
+    P = Y.shape[0]
+    if bits.dim() == 3 and bits.shape[0] != P:
+        raise ValueError("bits[P, M, ldw] and Y[P, N] disagree on P")
+    pstride = M * ldw if bits.dim() == 3 else 0
+    ldy = Y.stride(0) if P > 1 else max(Y.stride(0), N)
+    X = torch.empty(P, M, dtype=torch.float32, device=dev)
+    R = torch.empty(P, N, dtype=torch.float32, device=dev)
+    n_iter = torch.empty(P, dtype=torch.int32, device=dev)
+    ldt = max(max_iter, 1)
+    idx_trace = torch.empty(P, ldt, dtype=torch.int32, device=dev) if trace else None
+    c_trace = torch.empty(P, ldt, dtype=torch.float32, device=dev) if trace else None
+    if workspace is None:
+        workspace = torch.empty(lib.mp_workspace_bytes_signs_many(N, M, P) + 256, dtype=torch.uint8, device=dev)
+    base = workspace.data_ptr()
+    off = (-base) % 256
+    with torch.cuda.device(dev):
+        _check(lib.mp_recover_signs_many(bits.data_ptr(), N, M, ldw, pstride, float(scale), Y.data_ptr(), ldy, P, float(eps), int(max_iter),
+                                         X.data_ptr(), R.data_ptr(), n_iter.data_ptr(),
+                                         idx_trace.data_ptr() if trace else None, c_trace.data_ptr() if trace else None, ldt,
+                                         base + off, workspace.numel() - off, _stream_ptr(stream)))
+    return Recovered(X, R, n_iter, idx_trace, c_trace, workspace)
 
 
 def _host(t: torch.Tensor, dtype, what: str):

@@ -115,3 +115,16 @@ def test_argument_errors_of_mp_transpose_rowmajor():
     assert f(ok, 8, 8, 7, ok2, 8, None) == 1                                   # ldr < M
     assert f(ok, 8, 8, 8, ok2, 6, None) == 1                                   # ld < N / ld % 4
     assert f(ok, 8, 8, 8, C.c_void_p(4096 + 64), 8, None) == 1                 # overlapping buffers
+
+
+def test_argument_errors_of_mp_recover_signs_many():
+    from paper_0809_1833_b200.binding import lib
+    ok = C.c_void_p(4096)
+    f = lib.mp_recover_signs_many
+
+    def call(bits=ok, N=64, M=8, ldw=2, ps=16, scale=0.125, Y=ok, ldy=64, P=2, eps=0.1, T=4, X=ok, R=ok, n=ok, it=None, ct=None, ldt=4, ws=ok, wsb=256):
+        return f(bits, N, M, ldw, ps, scale, Y, ldy, P, eps, T, X, R, n, it, ct, ldt, ws, wsb, None)
+    assert call(bits=None) == 1 and call(P=0) == 1 and call(ldw=1) == 1 and call(ps=8) == 1 and call(scale=0.0) == 1
+    assert call(ldy=32) == 1 and call(T=-1) == 1 and call(eps=float("nan")) == 1 and call(it=ok, ldt=2) == 1
+    assert call(ws=None) == 4 and call(wsb=16) == 4
+    assert lib.mp_workspace_bytes_signs_many(8, 8, 0) == 0 and lib.mp_workspace_bytes_signs_many(8, 8, 3) == 256

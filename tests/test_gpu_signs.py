@@ -80,3 +80,63 @@ def test_cfg3_signs_sampled_grading(mp):
     grading.grade_sampled(pb.psi32, pb.Y[0], idx, cc, t, r, ts)
     assert set(idx.tolist()) == set(pb.S[0].tolist())
     assert np.linalg.norm(x - pb.X[0]) <= 1e-4 * np.linalg.norm(pb.X[0])
+
+
+# ------------------------------------------------------------------------------------------ many problems, one CTA each
+def run_signs_many(mp, pbs, eps, max_iter, shared=False):
+    M, N = pbs[0].psi32.shape
+    P = len(pbs)
+    ld = (N + 3) // 4 * 4
+    stack = torch.full((P * M, ld), 7.0, dtype=torch.float32, device="cuda")
+    for q, pb in enumerate(pbs):
+        stack[q * M:(q + 1) * M, :N] = dev(pb.psi32)
+    bits, scale, n_bad = mp.mp_pack_signs(stack[:, :N])                           # the P dictionaries packed as one stack
+    assert n_bad == 0
+    bits = bits.view(P, M, -1)
+    Y = dev(np.stack([pb.Y[0] for pb in pbs]))
+    res = mp.mp_recover_signs_many(bits[0] if shared else bits, N, scale, Y, eps, max_iter, trace=True)
+    torch.cuda.synchronize()
+    return res.x.cpu().numpy(), res.r.cpu().numpy(), res.n_iter.cpu().numpy(), res.idx_trace.cpu().numpy(), res.c_trace.cpu().numpy()
+
+
+@pytest.mark.parametrize("N,M,K,P", [(256, 1024, 16, 5), (100, 37, 4, 9), (500, 1000, 30, 4), (1000, 1000, 40, 3), (33, 150, 3, 200),
+                                     (1, 3, 1, 2), (2048, 300, 12, 2)])
+def test_signs_many_every_problem_graded_like_a_single_run(mp, N, M, K, P):
+    """Problem q's result must be MP on (expanded dictionary q, y_q): full grading of every problem against the oracle."""
+    cfg = problems.custom_config(N, M, K, dictionary="bernoulli", eps=1e-5, max_iter=8 * K)
+    pbs = [problems.make_problem(cfg, seed=20 + q) for q in range(P)]
+    if P > 4:
+        pbs[1].Y[0][:] = 0.0                                                       # one problem that stops at once
+    X, R, T, I, Cc = run_signs_many(mp, pbs, cfg.eps, cfg.max_iter)
+    if P > 4:
+        assert T[1] == 0 and not X[1].any()
+    for q, pb in enumerate(pbs):
+        t = int(T[q])
+        grading.grade_single(pb.psi32, pb.Y[0], cfg.eps, cfg.max_iter, X[q], R[q], t, I[q, :t], Cc[q, :t], nthreads=4)
+
+
+def test_signs_many_phase_diagram_cell_and_shared_dictionary(mp):
+    """A cell of the paper's Fig. 1 experiment with its own parameters (M = 1000, rho = 0.5, sigma = 0.03, U[-1,1] nonzeros,
+    eps = 1e-7, T = N): every trial graded and recovered (Eq. 14 ~ 0); then all signals against ONE shared dictionary."""
+    M, N, K, P = 1000, 500, 30, 4
+    cfg = problems.custom_config(N, M, K, dictionary="bernoulli", values="uniform", eps=1e-7, max_iter=N)
+    pbs = [problems.make_problem(cfg, seed=60 + q) for q in range(P)]
+    X, R, T, I, Cc = run_signs_many(mp, pbs, cfg.eps, cfg.max_iter)
+    for q, pb in enumerate(pbs):
+        t = int(T[q])
+        grading.grade_single(pb.psi32, pb.Y[0], cfg.eps, cfg.max_iter, X[q], R[q], t, I[q, :t], Cc[q, :t], nthreads=4)
+        assert oracle.reconstruction_error_pct(X[q].astype(np.float64), pb.X[0]) < 1e-6
+    cfgb = problems.custom_config(N, M, K, dictionary="bernoulli", values="uniform", eps=1e-7, max_iter=N, B=P)
+    pb = problems.make_problem(cfgb, 7)
+    shared = [problems.Problem(cfgb, pb.psi_raw, pb.psi32, pb.X[q:q + 1], pb.S[q:q + 1], pb.Y[q:q + 1]) for q in range(P)]
+    X, R, T, I, Cc = run_signs_many(mp, shared, cfgb.eps, cfgb.max_iter, shared=True)
+    for q in range(P):
+        t = int(T[q])
+        grading.grade_single(pb.psi32, pb.Y[q], cfgb.eps, cfgb.max_iter, X[q], R[q], t, I[q, :t], Cc[q, :t], nthreads=4)
+
+
+def test_signs_many_refuses_what_does_not_fit(mp):
+    bits = torch.zeros(1, 4096, 64, dtype=torch.int32, device="cuda")           # N = 2048, M = 4096: 1 MB of bits per problem
+    with pytest.raises(mp.MPError) as e:
+        mp.mp_recover_signs_many(bits, 2048, 1.0 / 45.0, torch.zeros(1, 2048, device="cuda"), 1e-5, 4)
+    assert e.value.status == mp.MP_ERR_UNSUPPORTED
