@@ -226,8 +226,9 @@ MP_API const char* mp_last_error(void);
  *                   copies through shared memory, 2 = stream loop of small kernels (general fallback; synchronises the
  *                   host every "chunk" iterations to read the stop flag), 3 = persistent cooperative kernel that streams
  *                   the dictionary into registers with 128-bit loads
- *   "l2_resident_mb" algo 3, dictionaries larger than L2: MB of rows loaded L2::evict_last so that they stay in L2 across
- *                   iterations (the rest is loaded evict_first); 0 = auto (68), 1 = off
+ *   "l2_resident_mb" algo 3 (and the float64 / Orthogonal MP kernels): MB of dictionary rows loaded L2::evict_last so that they
+ *                   stay in L2 across iterations (the rest is loaded evict_first); 0 = auto (68 MB for dictionaries above
+ *                   110 MB), 1 = off, other = that many MB for every dictionary larger than it
  *   "warps"         consumer warps per CTA of the persistent kernel (0 = auto)
  *   "slot_bytes"    bytes of one shared-memory stage (0 = auto);   "depth"  stages per warp (0 = auto)
  *   "grid"          CTAs of the persistent kernel (0 = auto = one per SM)

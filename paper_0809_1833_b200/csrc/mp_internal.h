@@ -51,12 +51,15 @@ struct Workspace {
 };
 size_t workspace_layout(int N, int M, int B, void* base, Workspace* ws);
 static inline int round_up(int v, int m) { return (v + m - 1) / m * m; }
-// L2 residency (mp_common.cuh): groups of rows per CTA to load with evict_last.  Only for dictionaries that do not fit in L2
-// anyway (> 72 MB); knob "l2_resident_mb": 0 = auto (68 MB, measured optimum on B200), 1 = off, else the MB to keep.
+// L2 residency (mp_common.cuh): groups of rows per CTA to load with evict_last.  Auto (knob "l2_resident_mb" = 0): 68 MB, the
+// measured optimum on B200, for dictionaries above 110 MB -- up to ~100 MB the plain LRU behaviour of the L2 already serves a
+// cyclic stream (84 MB: 9.3 us per iteration without hints, 10.5 us with) and above it the stream thrashes (134 MB: 22.2 us
+// without, 15.2 us with).  1 = off; any other value = that many MB, for every dictionary larger than it.
 static inline int l2_resident_groups(double dict_bytes, int grid, double group_bytes)
 {
-    const double target = options().l2_resident_mb == 0 ? 68e6 : options().l2_resident_mb == 1 ? 0.0 : 1e6 * (double)options().l2_resident_mb;
-    if (!(dict_bytes > 72e6) || !(target > 0.0) || grid < 1) return 0;
+    const int64_t knob = options().l2_resident_mb;
+    const double target = knob == 0 ? 68e6 : knob == 1 ? 0.0 : 1e6 * (double)knob;
+    if (!(target > 0.0) || grid < 1 || !(dict_bytes > (knob == 0 ? 110e6 : target))) return 0;
     return (int)(target / grid / group_bytes);
 }
 

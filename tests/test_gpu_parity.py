@@ -428,3 +428,21 @@ def test_solve_from_the_papers_layout(mp):
     g = grading.grade_single(pb.psi32, pb.Y[0], c.eps, c.max_iter, res.x.cpu().numpy(), res.r.cpu().numpy(), t,
                              res.idx_trace.cpu().numpy()[:t], res.c_trace.cpu().numpy()[:t], x_true=pb.X[0], support=pb.S[0])
     assert g.exact_recovery
+
+
+@pytest.mark.parametrize("N,M,K", [(1002, 19000, 40), (300, 64000, 24)])
+def test_l2_residency_hints_do_not_change_results(mp, N, M, K):
+    """The L2::evict_last / evict_first loads of the register-streaming kernel (auto for dictionaries above 110 MB; forced here
+    on 76 MB ones with the knob): ragged N, full grading, and bit-identical results with the hints switched off."""
+    cfg = problems.custom_config(N, M, K, eps=1e-5, max_iter=6 * K)
+    pb = problems.make_problem(cfg, seed=9)
+    mp.mp_set_int("l2_resident_mb", 40)
+    try:
+        out = run_single(mp, pb.psi32, pb.Y[0], cfg.eps, cfg.max_iter, 3)
+        grading.grade_single(pb.psi32, pb.Y[0], cfg.eps, cfg.max_iter, *out, x_true=pb.X[0], support=pb.S[0])
+        mp.mp_set_int("l2_resident_mb", 1)
+        off = run_single(mp, pb.psi32, pb.Y[0], cfg.eps, cfg.max_iter, 3)
+    finally:
+        mp.mp_set_int("l2_resident_mb", 0)
+    for a, b in zip(out, off):
+        assert np.array_equal(a, b)
