@@ -201,3 +201,15 @@ def test_long_residual_falls_back_to_single_signal_solves(mp):
     out = run_many(mp, pbs, cfg.eps, cfg.max_iter)
     assert mp.mp_get_int("info_many_cluster") == 0
     grade_all(pbs, cfg.eps, cfg.max_iter, out)
+
+
+def test_repeated_runs_are_bit_identical(mp):
+    """Race detector of last resort (compute-sanitizer is not available on the pool): the exchange is st.async + mbarrier with
+    alternating slots, the problems are drawn from a device counter -- 25 runs of a 150-problem batch, in three plans, must give
+    the same bits every time (a lost or stale key, or a slot overwritten too early, shows up as a different trace)."""
+    cfg, pbs = make_many(96, 400, 6, 150, eps=1e-5, max_iter=40)
+    for cluster, stat in ((0, 0), (16, 0), (4, 2)):
+        ref = run_many(mp, pbs, cfg.eps, cfg.max_iter, cluster=cluster, stat=stat)
+        for _ in range(24):
+            assert _traces_equal(ref, run_many(mp, pbs, cfg.eps, cfg.max_iter, cluster=cluster, stat=stat))
+    grade_all(pbs[:20], cfg.eps, cfg.max_iter, tuple(a[:20] for a in ref))
