@@ -208,7 +208,7 @@ MP_API mp_status mp_recover_signs_many(const uint32_t* bits, int N, int M, int64
  * when it fits (<= ~3.5 MB), else streamed from L2; the argmax is exchanged through distributed shared memory with one
  * hardware cluster barrier per iteration; clusters draw problems from a device counter.  N > 2048 falls back to one
  * single-signal solve after another.  Knobs: "many_cluster" (CTAs per problem, 0 = auto), "many_threads", "many_stat"
- * (2 = never stationary).  Workspace: mp_workspace_bytes_many(N, M, P). */
+ * (2 = never stationary), "many_l2_mb" (MB of dictionaries the plan keeps in flight, 0 = auto = 64).  Workspace: mp_workspace_bytes_many(N, M, P). */
 MP_API size_t mp_workspace_bytes_many(int N, int M, int P);
 MP_API mp_status mp_recover_many(const float* psi_t, int N, int M, int64_t ld, int64_t problem_stride,
                           const float* Y, int64_t ldy, int P, float eps, int max_iter,

@@ -139,6 +139,7 @@ static int64_t* option_slot(const char* name)
     if (!strcmp(name, "many_cluster")) return &o.many_cluster;
     if (!strcmp(name, "many_threads")) return &o.many_threads;
     if (!strcmp(name, "many_stat")) return &o.many_stat;
+    if (!strcmp(name, "many_l2_mb")) return &o.many_l2_mb;
     if (!strcmp(name, "info_many_cluster")) return &o.info_many_cluster;
     if (!strcmp(name, "info_many_stat")) return &o.info_many_stat;
     if (!strcmp(name, "info_many_clusters")) return &o.info_many_clusters;

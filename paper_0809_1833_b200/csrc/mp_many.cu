@@ -509,7 +509,8 @@ static mp_status many_plan_and_launch(ManyParams p, const DeviceInfo& di, cudaSt
 {
     const Options& o = options();
     const double bytes = 4.0 * p.N * p.M;
-    int64_t qt = p.pstride == 0 ? p.P : (int64_t)(64e6 / bytes);               // one shared dictionary: its footprint does not grow
+    const double l2_budget = o.many_l2_mb > 0 ? 1e6 * (double)o.many_l2_mb : 64e6;   // dictionaries in flight stay L2-resident
+    int64_t qt = p.pstride == 0 ? p.P : (int64_t)(l2_budget / bytes);               // one shared dictionary: its footprint does not grow
     if (qt < 1) qt = 1;
     if (qt > p.P) qt = p.P;
     int c_cap = 1;
