@@ -48,6 +48,15 @@ __device__ __forceinline__ double warp_sum(double v)
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
     return v;
 }
+// 64-bit max over the warp with two hardware reductions (REDUX): the high words first, then the low words of the lanes that hold
+// the winning high word.  Same result as the butterfly below in a fifth of the latency.
+__device__ __forceinline__ unsigned long long warp_max_redux(unsigned long long k)
+{
+    const unsigned int hi = (unsigned int)(k >> 32);
+    const unsigned int m = __reduce_max_sync(0xffffffffu, hi);
+    const unsigned int lo = __reduce_max_sync(0xffffffffu, hi == m ? (unsigned int)k : 0u);
+    return ((unsigned long long)m << 32) | lo;
+}
 __device__ __forceinline__ unsigned long long warp_max(unsigned long long v)
 {
 #pragma unroll

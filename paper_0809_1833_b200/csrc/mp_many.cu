@@ -62,15 +62,6 @@ __device__ __forceinline__ float4 many_ldg_cg4(const float4* p)
     return v;
 }
 
-// 64-bit max over the warp with two hardware reductions (REDUX): the high words first, then the low words of the lanes
-// that hold the winning high word.  Real keys have a non-zero low word, so 0 stays "empty".
-__device__ __forceinline__ unsigned long long warp_max_redux(unsigned long long k)
-{
-    const unsigned int hi = (unsigned int)(k >> 32);
-    const unsigned int m = __reduce_max_sync(0xffffffffu, hi);
-    const unsigned int lo = __reduce_max_sync(0xffffffffu, hi == m ? (unsigned int)k : 0u);
-    return ((unsigned long long)m << 32) | lo;
-}
 // shared::cluster address of `saddr` (a shared::cta address) in CTA `rank` of the cluster
 __device__ __forceinline__ uint32_t mapa_u32(uint32_t saddr, uint32_t rank)
 {

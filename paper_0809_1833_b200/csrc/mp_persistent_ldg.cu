@@ -64,6 +64,8 @@ mp_persistent_ldg_kernel(const LdgParams p)
     unsigned long long* skey = reinterpret_cast<unsigned long long*>(red + kLdgMaxWarps);
     float* part = reinterpret_cast<float*>(skey + 2);                          // [atom of this CTA][chunk] partial dots
 
+    if (tid < kLdgMaxWarps) red[tid] = 0.0;                                     // partial sums of absent warps stay 0
+    __syncthreads();
     const int a0 = (int)(((int64_t)blockIdx.x * p.M) / G);
     const int a1 = (int)(((int64_t)(blockIdx.x + 1) * p.M) / G);
     const int n_atoms = a1 - a0;
@@ -86,8 +88,7 @@ mp_persistent_ldg_kernel(const LdgParams p)
     __syncthreads();
     double rr = 0.0;
     for (int w = 0; w < W; w++) rr += red[w];
-    const double yy = rr;
-    const double thresh = (double)p.eps * sqrt(yy);
+    const double thresh2 = ((double)p.eps * (double)p.eps) * rr;                // ||r|| > eps ||y||  <=>  ||r||^2 > eps^2 ||y||^2
     __syncthreads();
 
     const float4* r4 = reinterpret_cast<const float4*>(r32);
@@ -129,7 +130,7 @@ mp_persistent_ldg_kernel(const LdgParams p)
     if (have) load_item(it);
     int t = 0;
     // ---- the loop: while ||r|| > eps ||y|| and t < T -----------------------------------------------------------
-    while ((sqrt(rr) > thresh) && (t < p.max_iter)) {
+    while ((rr > thresh2) && (t < p.max_iter)) {
         // ---------- Eq. 9: items = (group of A atoms, chunk of 32*UC float4), dealt round-robin to the warps --------------
         // One item is always in flight per warp: `v` was loaded before the previous iteration's barrier (or in the
         // prologue), so the stream does not drain while the CTAs meet and update the residual.
@@ -180,14 +181,14 @@ mp_persistent_ldg_kernel(const LdgParams p)
             const unsigned long long k = pack_key(c, a0 + a);
             best = k > best ? k : best;
         }
-        best = warp_max(best);
+        best = warp_max_redux(best);
 
         // ---------- block argmax -> grid argmax, ONE grid barrier -------------------------------------------------
         if (lane == 0) wkey[warp] = best;
         __syncthreads();
         if (warp == 0) {
             unsigned long long k = lane < W ? wkey[lane] : 0ull;
-            k = warp_max(k);
+            k = warp_max_redux(k);
             if (lane == 0) {
                 unsigned long long* slot_key = p.ctrl + 1 + (t % 3);
                 if (k) red_max_u64(slot_key, k);
@@ -227,21 +228,25 @@ mp_persistent_ldg_kernel(const LdgParams p)
             if (lane == 0) red[warp] = s2;
         }
         // ---------- Eq. 10, Eq. 12, traces: CTA 0 only ---------------------------------------------------------------
-        if (blockIdx.x == 0 && tid == 0) {
+        if (blockIdx.x == 0 && tid == THREADS - 32) {                          // not the thread every CTA's barrier waits for
             red_add_f64(p.x64 + i, cd);
             if (p.idx_trace) p.idx_trace[t] = i;
             if (p.c_trace) p.c_trace[t] = c;
             st_relaxed_u64(p.ctrl + 1 + ((t + 2) % 3), 0ull);                   // slot of iteration t-1: everyone has read it
         }
         __syncthreads();
-        rr = 0.0;
-        for (int w = 0; w < W; w++) rr += red[w];
+        {                                                                       // W <= 16 partials (absent warps hold 0), fixed tree
+            const double2* r2 = reinterpret_cast<const double2*>(red);
+            const double2 q0 = r2[0], q1 = r2[1], q2 = r2[2], q3 = r2[3], q4 = r2[4], q5 = r2[5], q6 = r2[6], q7 = r2[7];
+            rr = (((q0.x + q0.y) + (q1.x + q1.y)) + ((q2.x + q2.y) + (q3.x + q3.y))) +
+                 (((q4.x + q4.y) + (q5.x + q5.y)) + ((q6.x + q6.y) + (q7.x + q7.y)));
+        }
         t += 1;
     }
 
     // ---- P:86 return x~ (and r, t): CTA 0 -------------------------------------------------------------------------------
     if (blockIdx.x == 0) {
-        if (tid == 0) __threadfence();
+        __threadfence();                                                        // the x~ accumulations of this CTA (thread THREADS - 32)
         __syncthreads();
         for (int m = tid; m < p.M; m += THREADS) p.x[m] = (float)__ldcg(p.x64 + m);
         for (int n = tid; n < p.N; n += THREADS) p.r[n] = r32[n];

@@ -100,14 +100,14 @@ mp_persistent_signs_kernel(const SignParams p)
     __syncthreads();
     double rr = 0.0;
     for (int w = 0; w < W; w++) rr += red[w];
-    const double thresh = (double)p.eps * sqrt(rr);
+    const double thresh2 = ((double)p.eps * (double)p.eps) * rr;                // ||r|| > eps ||y||  <=>  ||r||^2 > eps^2 ||y||^2
     __syncthreads();
 
     const int n_items = p.AG * p.WP;
     const double dscale = (double)p.scale;
     int t = 0;
     // ---- the loop: while ||r|| > eps ||y|| and t < T -----------------------------------------------------------
-    while ((sqrt(rr) > thresh) && (t < p.max_iter)) {
+    while ((rr > thresh2) && (t < p.max_iter)) {
         // ---------- table of the 16 signed sums of every four residual values -----------------------------------------------
         for (int e = tid; e < 4 * p.Nr; e += THREADS) {
             const int g = e >> 4, nib = e & 15;
@@ -149,12 +149,12 @@ mp_persistent_signs_kernel(const SignParams p)
             const unsigned long long k = pack_key(p.scale * c, a0 + a);
             best = k > best ? k : best;
         }
-        best = warp_max(best);
+        best = warp_max_redux(best);
         if (lane == 0) wkey[warp] = best;
         __syncthreads();
         if (warp == 0) {
             unsigned long long k = lane < W ? wkey[lane] : 0ull;
-            k = warp_max(k);
+            k = warp_max_redux(k);
             if (lane == 0) {
                 unsigned long long* slot_key = p.ctrl + 1 + (t % 3);
                 if (k) red_max_u64(slot_key, k);
@@ -185,7 +185,7 @@ mp_persistent_signs_kernel(const SignParams p)
             s2 = warp_sum(s2);
             if (lane == 0) red[warp] = s2;
         }
-        if (blockIdx.x == 0 && tid == 0) {
+        if (blockIdx.x == 0 && tid == THREADS - 32) {                          // not the thread every CTA's barrier waits for
             red_add_f64(p.x64 + i, cd);
             if (p.idx_trace) p.idx_trace[t] = i;
             if (p.c_trace) p.c_trace[t] = c;
@@ -198,7 +198,7 @@ mp_persistent_signs_kernel(const SignParams p)
     }
 
     if (blockIdx.x == 0) {
-        if (tid == 0) __threadfence();
+        __threadfence();
         __syncthreads();
         for (int m = tid; m < p.M; m += THREADS) p.x[m] = (float)__ldcg(p.x64 + m);
         for (int n = tid; n < p.N; n += THREADS) p.r[n] = r32[n];

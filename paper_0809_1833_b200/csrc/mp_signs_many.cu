@@ -37,14 +37,6 @@ struct SignManyParams {
     int max_iter;
 };
 
-__device__ __forceinline__ unsigned long long sm_warp_max(unsigned long long k)
-{
-    const unsigned int hi = (unsigned int)(k >> 32);
-    const unsigned int m = __reduce_max_sync(0xffffffffu, hi);
-    const unsigned int lo = __reduce_max_sync(0xffffffffu, hi == m ? (unsigned int)k : 0u);
-    return ((unsigned long long)m << 32) | lo;
-}
-
 __global__ void __launch_bounds__(kSmThreads, 1)
 mp_many_signs_kernel(const SignManyParams p)
 {
@@ -142,10 +134,10 @@ mp_many_signs_kernel(const SignManyParams p)
                     best = k > best ? k : best;
                 }
             }
-            best = sm_warp_max(best);
+            best = warp_max_redux(best);
             if (lane == 0) wkey[warp] = best;
             __syncthreads();
-            const unsigned long long key = sm_warp_max(lane < kSmWarps ? wkey[lane] : 0ull);
+            const unsigned long long key = warp_max_redux(lane < kSmWarps ? wkey[lane] : 0ull);
             const int i = key_index(key);
             const float c = key_value(key);
             const double cd = (double)c;
