@@ -72,7 +72,7 @@ MP_API mp_status mp_normalize_columns(float* psi_t, int N, int M, int64_t ld, fl
 /* Ingestion of the paper's own layout.  The listings hold Psi ROW-MAJOR, psi[n*ldr + m] (A2 P:360,
  * P:424; ldr >= M, any alignment), which makes every atom a stride-M gather (the axpy column of A2 P:470); this copies it once
  * into the atom-major psi_t[m*ld + n] every other entry point takes (ld >= N, ld % 4 == 0, 16-byte aligned).  Out of place
- * (overlapping buffers are refused), bit-exact, HBM-bound (8NM bytes); elements psi_t[m*ld + n], n >= N, are not written. */
+ * (overlapping buffers are refused), bit-exact, HBM-bound (8NM bytes; 128-bit accesses when psi is 16-byte aligned and ldr % 4 == 0); elements psi_t[m*ld + n], n >= N, are not written. */
 MP_API mp_status mp_transpose_rowmajor(const float* psi, int N, int M, int64_t ldr, float* psi_t, int64_t ld, void* stream);
 
 /* The MP loop above for one signal.

@@ -182,7 +182,7 @@ __device__ __forceinline__ double2 ldg_cg_d2_hint(const double2* p, uint64_t pol
 // group g of n_groups is one of the rg resident ones (spread evenly: L2 hits and HBM misses interleave in time)
 __device__ __forceinline__ bool l2_group_is_resident(int g, int rg, int n_groups)
 {
-    return ((g + 1) * rg) / n_groups != (g * rg) / n_groups;
+    return ((long long)(g + 1) * rg) / n_groups != ((long long)g * rg) / n_groups;
 }
 
 }  // namespace mp

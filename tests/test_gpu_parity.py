@@ -397,15 +397,18 @@ def test_host_entry_point_matches_device_entry_point(mp):
 
 
 # ------------------------------------------------------------------------------------------ the paper's row-major layout
-@pytest.mark.parametrize("N,M,ldr", [(256, 1024, None), (250, 333, 340), (1, 5, None), (4096, 300, None), (37, 1000, 1003), (65, 129, None)])
-def test_rowmajor_ingestion_is_bit_exact(mp, N, M, ldr):
+@pytest.mark.parametrize("aligned", [False, True])
+@pytest.mark.parametrize("N,M,ldr", [(256, 1024, None), (250, 333, 340), (1, 5, None), (4096, 300, None), (37, 1000, 1003), (65, 129, None),
+                                     (130, 250, 252), (63, 67, 68)])
+def test_rowmajor_ingestion_is_bit_exact(mp, N, M, ldr, aligned):
     """mp_transpose_rowmajor against the oracle's element-by-element definition (A2 P:360 layout -> atom-major): bit-exact,
     pad columns of the destination untouched, odd source strides and unaligned source pointers accepted."""
     rng = np.random.default_rng(N * 1000 + M)
     psi = rng.standard_normal((N, M)).astype(np.float32)
     ldr = ldr or M
+    off = 0 if aligned else 1                                                      # 16-byte aligned (128-bit kernel if ldr % 4 == 0) or not
     src = torch.full((N * ldr + 1,), -3.0, dtype=torch.float32, device="cuda")
-    src_v = src[1:].view(N, ldr)[:, :M]                                            # 4-byte aligned only
+    src_v = src[off:off + N * ldr].view(N, ldr)[:, :M]
     src_v.copy_(dev(psi))
     ld = (N + 3) // 4 * 4 + 4
     dst = torch.full((M, ld), 7.0, dtype=torch.float32, device="cuda")
