@@ -201,6 +201,13 @@ def main():
                          "problems each with its own Bernoulli dictionary, eps=1e-7, T=N, solved by one mp_recover_many launch")
     ap.add_argument("--knob", action="append", default=[], metavar="NAME=VALUE", help="mp_set_int knob (profiling runs)")
     args = ap.parse_args()
+    if args.config == "cfg4":
+        # the size sweep of BASELINE.json configs[3]: one full bench line per dictionary size (4 MiB ... 1 GiB), each from a
+        # fresh process so that no state carries over between sizes
+        for m in (2048, 4096, 8192, 16384, 32768):
+            argv = [a if a != "cfg4" else "cfg4_%d" % m for a in sys.argv[1:]]
+            subprocess.run([sys.executable, os.path.abspath(__file__)] + argv, check=True)
+        return
     cfg = synth.config(args.config)
     if args.max_iter is not None:
         cfg = synth.Config(**{**cfg.__dict__, "max_iter": args.max_iter})
