@@ -229,6 +229,8 @@ MP_API const char* mp_last_error(void);
  *   "l2_resident_mb" algo 3 (and the float64 / Orthogonal MP kernels): MB of dictionary rows loaded L2::evict_last so that they
  *                   stay in L2 across iterations (the rest is loaded evict_first); 0 = auto (68 MB for dictionaries above
  *                   110 MB), 1 = off, other = that many MB for every dictionary larger than it
+ *   "l2_demote"     0 (default) = when a solve ends the pinned rows are handed back (applypriority L2::evict_normal), so later
+ *                   kernels find a normal L2; 1 = left as they are (measurements)
  *   "warps"         consumer warps per CTA of the persistent kernel (0 = auto)
  *   "slot_bytes"    bytes of one shared-memory stage (0 = auto);   "depth"  stages per warp (0 = auto)
  *   "grid"          CTAs of the persistent kernel (0 = auto = one per SM)

@@ -185,4 +185,14 @@ __device__ __forceinline__ bool l2_group_is_resident(int g, int rg, int n_groups
     return ((long long)(g + 1) * rg) / n_groups != ((long long)g * rg) / n_groups;
 }
 
+// At the end of a solve the rows that were pinned with evict_last are handed back: `applypriority ... L2::evict_normal` (SASS
+// CCTL.E.DML2) on every 128-byte line of a row, so that kernels running afterwards find an L2 without 68 MB of lines they cannot
+// displace.  `row` .. `row + bytes` is covered from the enclosing 128-byte boundary; one warp per row, lanes stride the lines.
+__device__ __forceinline__ void l2_demote_row(const void* row, size_t bytes, int lane)
+{
+    const uintptr_t first = reinterpret_cast<uintptr_t>(row) & ~(uintptr_t)127, last = reinterpret_cast<uintptr_t>(row) + bytes;
+    for (uintptr_t a = first + (uintptr_t)lane * 128; a < last; a += 32 * 128)
+        asm volatile("applypriority.global.L2::evict_normal [%0], 128;" ::"l"(a) : "memory");
+}
+
 }  // namespace mp

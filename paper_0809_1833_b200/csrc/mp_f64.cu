@@ -36,6 +36,7 @@ struct F64Params {
     int N, M, Npad, Nr;         // Npad = N rounded up to 2, Nr = N rounded up to 128
     double eps;
     int max_iter;
+    int demote;                 // hand the pinned rows back at the end (knob l2_demote, default on)
     int resident_groups;        // groups of A atoms per CTA loaded L2::evict_last (mp_common.cuh), 0 = no hints
 };
 
@@ -239,6 +240,16 @@ mp_persistent_f64_kernel(const F64Params p)
         t += 1;
     }
 
+    // ---- hand the pinned rows back to the L2's normal replacement (see l2_demote_row) ------------------------------------------
+    if (A <= 4 && p.resident_groups > 0 && p.demote) {
+        for (int g = warp; g < n_groups; g += W) {
+            if (!l2_group_is_resident(g, p.resident_groups, n_groups)) continue;
+            for (int a = 0; a < A; a++) {
+                const int rel = g * A + a < n_atoms ? g * A + a : n_atoms - 1;
+                l2_demote_row(p.psi_t + (int64_t)(a0 + rel) * p.ld, (size_t)p.Npad * 8, lane);
+            }
+        }
+    }
     // ---- P:86 return x~ (and r, t): CTA 0 -------------------------------------------------------------------------------
     if (blockIdx.x == 0) {
         if (tid == 0) __threadfence();
@@ -375,6 +386,7 @@ MP_API mp_status mp_recover_f64(const double* psi_t, int N, int M, int64_t ld,
     p.slots = reinterpret_cast<Cand*>(base + 256 + (sizeof(double) * (size_t)M + 255) / 256 * 256);
     p.ld = ld; p.N = N; p.M = M; p.Npad = round_up(N, 2); p.Nr = round_up(N, 128);
     p.eps = eps; p.max_iter = max_iter;
+    p.demote = options().l2_demote != 1;
     p.resident_groups = l2_resident_groups(8.0 * (double)ld * M, plan.grid, 8.0 * (double)ld * plan.A);
     if (plan.A == 16) return launch_f64<16, 1>(p, plan, di.device, s);
     if (plan.A == 8) return launch_f64<8, 2>(p, plan, di.device, s);

@@ -31,6 +31,7 @@ struct OmpPParams {
     int SLp;                    // padded (odd) pitch of a basis-vector slice in shared memory
     int atoms_max;
     float eps;
+    int demote;                 // hand the pinned rows back at the end (knob l2_demote, default on)
     int resident_groups;        // groups of A atoms per CTA loaded L2::evict_last (mp_common.cuh), 0 = no hints
 };
 
@@ -321,6 +322,16 @@ mp_omp_persistent_kernel(const OmpPParams p)
         t += 1;
     }
 
+    // ---- hand the pinned rows back to the L2's normal replacement (see l2_demote_row) ------------------------------------------
+    if (A <= 4 && p.resident_groups > 0 && p.demote) {
+        for (int g = warp; g < n_groups; g += W) {
+            if (!l2_group_is_resident(g, p.resident_groups, n_groups)) continue;
+            for (int a = 0; a < A; a++) {
+                const int rel = g * A + a < n_atoms ? g * A + a : n_atoms - 1;
+                l2_demote_row(p.psi_t + (int64_t)(a0 + rel) * p.ld, (size_t)p.Npad * 4, lane);
+            }
+        }
+    }
     // ---- the state the back-substitution kernel needs: r (float64) and t ----------------------------------------------------------
     if (b == 0) {
         for (int n = tid; n < p.N; n += THREADS) ws.r64[n] = r64[n];
@@ -403,6 +414,7 @@ mp_status launch_omp_persistent(const OmpArgs& a, const OmpWs& ws, cudaStream_t 
     p.psi_t = a.psi_t; p.y = a.y; p.idx_trace = a.idx_trace; p.ws = ws; p.ld = a.ld;
     p.N = a.N; p.M = a.M; p.Npad = round_up(a.N, 4); p.Nr = round_up(a.N, 128); p.T = a.T; p.Tld = round_up(a.T, 32);
     p.SLp = plan.SLp; p.atoms_max = plan.atoms_max; p.eps = a.eps;
+    p.demote = options().l2_demote != 1;
     p.resident_groups = l2_resident_groups(4.0 * (double)a.ld * a.M, plan.grid, 4.0 * (double)a.ld * plan.A);
     if (plan.A == 16) return launch_omp_p<16, 1>(p, plan, di.device, stream);
     if (plan.A == 8) return launch_omp_p<8, 2>(p, plan, di.device, stream);

@@ -37,6 +37,7 @@ struct LdgParams {
     int N, M, Npad, Nr;
     float eps;
     int max_iter;
+    int demote;                 // hand the pinned rows back at the end (knob l2_demote, default on)
     int resident_groups;        // groups of A atoms per CTA loaded with L2::evict_last (0 = no residency hints)
 };
 
@@ -244,6 +245,16 @@ mp_persistent_ldg_kernel(const LdgParams p)
         t += 1;
     }
 
+    // ---- hand the pinned rows back to the L2's normal replacement (see l2_demote_row) ------------------------------------------
+    if (A <= 4 && p.resident_groups > 0 && p.demote) {
+        for (int g = warp; g < n_groups; g += W) {
+            if (!l2_group_is_resident(g, p.resident_groups, n_groups)) continue;
+            for (int a = 0; a < A; a++) {
+                const int rel = g * A + a < n_atoms ? g * A + a : n_atoms - 1;
+                l2_demote_row(p.psi_t + (int64_t)(a0 + rel) * p.ld, (size_t)p.Npad * 4, lane);
+            }
+        }
+    }
     // ---- P:86 return x~ (and r, t): CTA 0 -------------------------------------------------------------------------------
     if (blockIdx.x == 0) {
         __threadfence();                                                        // the x~ accumulations of this CTA (thread THREADS - 32)
@@ -332,6 +343,7 @@ mp_status launch_recover_persistent_ldg(const RecoverArgs& a, const Workspace& w
     p.N = a.N; p.M = a.M; p.Npad = round_up(a.N, 4); p.Nr = round_up(a.N, 128);
     p.eps = a.eps; p.max_iter = a.max_iter;
     // L2 residency: only for dictionaries that do not fit in L2 anyway.  Knob "l2_resident_mb": 0 = auto (68 MB), 1 = off.
+    p.demote = options().l2_demote != 1;
     p.resident_groups = l2_resident_groups(4.0 * (double)a.ld * a.M, plan.grid, 4.0 * (double)a.ld * plan.A);
     if (plan.A == 16) return launch_ldg<16, 1>(p, plan, di.device, stream);
     if (plan.A == 8) return launch_ldg<8, 2>(p, plan, di.device, stream);
