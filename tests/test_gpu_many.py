@@ -213,3 +213,30 @@ def test_repeated_runs_are_bit_identical(mp):
         for _ in range(24):
             assert _traces_equal(ref, run_many(mp, pbs, cfg.eps, cfg.max_iter, cluster=cluster, stat=stat))
     grade_all(pbs[:20], cfg.eps, cfg.max_iter, tuple(a[:20] for a in ref))
+
+
+def test_random_shapes_against_the_oracle(mp):
+    """A fixed-seed sweep over awkward shapes (N around the 128-float register classes, tiny and odd M, NaN in the pad columns
+    of the dictionary), three plans each: every problem fully graded."""
+    rng = np.random.default_rng(123)
+    for trial in range(14):
+        N = int(rng.choice([1, 3, 31, 33, 127, 129, 257, 385, 500, 641, 777, 1025, 1281, 1793, 2047]))
+        M = int(rng.choice([1, 2, 15, 17, 33, 100, 255, 300, 1000]))
+        if 4 * N * M > 4e6:
+            M = max(1, int(4e6 / (4 * N)))
+        K = max(1, min(M, N // 6 + 1, 10))
+        P = int(rng.choice([1, 3, 9]))
+        cfg = problems.custom_config(N, M, K, dictionary="bernoulli" if trial % 3 == 0 else "gaussian", eps=1e-5, max_iter=4 * K + 2)
+        pbs = [problems.make_problem(cfg, 2000 + 7 * trial + q) for q in range(P)]
+        ld = (N + 3) // 4 * 4 + 4 * (trial % 2)
+        buf = torch.full((P, M, ld), float("nan"), dtype=torch.float32, device="cuda")
+        for q, pb in enumerate(pbs):
+            buf[q, :, :N] = dev(pb.psi32)
+        Y = dev(np.stack([pb.Y[0] for pb in pbs]))
+        for knobs in ({}, {"many_stat": 2}, {"many_cluster": int(rng.choice([1, 2, 4, 8, 16]))}):
+            for k in ("many_stat", "many_cluster", "many_threads"):
+                mp.mp_set_int(k, knobs.get(k, 0))
+            res = mp.mp_recover_many(buf[:, :, :N], Y, cfg.eps, cfg.max_iter, trace=True)
+            torch.cuda.synchronize()
+            out = tuple(a.cpu().numpy() for a in (res.x, res.r, res.n_iter, res.idx_trace, res.c_trace))
+            grade_all(pbs, cfg.eps, cfg.max_iter, out)

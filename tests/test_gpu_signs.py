@@ -140,3 +140,28 @@ def test_signs_many_refuses_what_does_not_fit(mp):
     with pytest.raises(mp.MPError) as e:
         mp.mp_recover_signs_many(bits, 2048, 1.0 / 45.0, torch.zeros(1, 2048, device="cuda"), 1e-5, 4)
     assert e.value.status == mp.MP_ERR_UNSUPPORTED
+
+
+def test_signs_many_random_shapes_and_repeatability(mp):
+    """Fixed-seed sweep over awkward shapes (word boundaries of N, tiny M, more problems than SMs) with full grading, and 10 repeated
+    runs of a 300-problem batch giving the same bits (problems are drawn from a device counter)."""
+    rng = np.random.default_rng(77)
+    for trial in range(8):
+        N = int(rng.choice([1, 31, 32, 33, 64, 95, 129, 500, 1000, 1537]))
+        M = int(rng.choice([1, 2, 31, 33, 100, 511, 700]))
+        if N * M // 8 > 150000:
+            M = 150000 * 8 // N
+        K = max(1, min(M, N // 6 + 1, 8))
+        cfg = problems.custom_config(N, M, K, dictionary="bernoulli", eps=1e-5, max_iter=4 * K + 2)
+        pbs = [problems.make_problem(cfg, 3000 + 5 * trial + q) for q in range(int(rng.choice([1, 4, 11])))]
+        X, R, T, I, Cc = run_signs_many(mp, pbs, cfg.eps, cfg.max_iter)
+        for q, pb in enumerate(pbs):
+            t = int(T[q])
+            grading.grade_single(pb.psi32, pb.Y[0], cfg.eps, cfg.max_iter, X[q], R[q], t, I[q, :t], Cc[q, :t], nthreads=4)
+    cfg = problems.custom_config(96, 200, 5, dictionary="bernoulli", eps=1e-5, max_iter=30)
+    pbs = [problems.make_problem(cfg, 4000 + q) for q in range(300)]
+    ref = run_signs_many(mp, pbs, cfg.eps, cfg.max_iter)
+    for _ in range(9):
+        out = run_signs_many(mp, pbs, cfg.eps, cfg.max_iter)
+        assert np.array_equal(ref[0], out[0]) and np.array_equal(ref[1], out[1]) and np.array_equal(ref[2], out[2])
+        assert all(np.array_equal(ref[3][q, :ref[2][q]], out[3][q, :ref[2][q]]) for q in range(300))
