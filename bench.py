@@ -346,7 +346,7 @@ def main():
         e2e = {"value": its_e / dt_max, "unit": UNIT,
                "h2d_bytes_per_step": 4 * N * M + 4 * N, "d2h_bytes_per_step": 4 * M + 4 * N + 4,
                "ms_per_step": 1e3 * dt_max / args.steps,
-               "note": "mp_recover_host: cudaMalloc + H2D(Psi, y) + normalise + solve + D2H(x, r, n_iter) + free per step"}
+               "note": "mp_recover_host: stream-ordered device allocations + H2D(Psi, y) + normalise + solve + D2H(x, r, n_iter) + free per step"}
 
     if not args.no_e2e and B > 1:
         hp = torch.from_numpy(psi_raw).pin_memory(); hY = torch.from_numpy(Y).pin_memory()
@@ -361,7 +361,7 @@ def main():
         e2e = {"value": its_e / dt_max, "unit": UNIT,
                "h2d_bytes_per_step": 4 * N * M + 4 * N * B, "d2h_bytes_per_step": 4 * M * B + 4 * N * B + 4 * B,
                "ms_per_step": 1e3 * dt_max / args.steps,
-               "note": "mp_recover_batched_host: cudaMalloc + H2D(Psi, Y) + normalise + solve + D2H(X, R, n_iter) + free per step"}
+               "note": "mp_recover_batched_host: stream-ordered device allocations + H2D(Psi, Y) + normalise + solve + D2H(X, R, n_iter) + free per step"}
 
     if rank == 0:
         cb = None

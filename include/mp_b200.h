@@ -248,7 +248,8 @@ MP_API mp_status mp_get_int(const char* name, int64_t* value);
 MP_API int64_t mp_launch_count(void);
 
 /* ---- HOST-buffer entry points (end-to-end convenience; every pointer below is a HOST pointer) ----------
- * mp_recover_host allocates device buffers, copies psi_t (M*ld floats) and y to the device on an internal
+ * mp_recover_host allocates device buffers (stream-ordered, from the device's default memory pool, whose release threshold it
+ * raises so that the next call reuses them), copies psi_t (M*ld floats) and y to the device on an internal
  * stream, optionally normalises the columns on the device (normalize != 0; the host copy of psi_t is not
  * modified), runs mp_recover, copies x, r, n_iter (and the traces if non-null) back, synchronises and frees.
  * Pinned host memory makes the copies faster but is not required.  mp_recover_batched_host likewise. */
