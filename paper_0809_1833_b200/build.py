@@ -50,7 +50,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
             failed = True
     if failed:
         raise RuntimeError("nvcc failed")
-    subprocess.run([NVCC, "-shared", "-o", LIB + ".tmp", *objs, "-cudart", "static"], check=True)
+    subprocess.run([NVCC, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB + ".tmp", *objs, "-cudart", "static"], check=True)
     os.replace(LIB + ".tmp", LIB)
     return LIB
 
