@@ -14,9 +14,10 @@
  * over a dictionary Psi (N x M) whose columns psi_m have unit l2 norm (Eq. 4).
  *
  * CONVENTIONS (all entry points unless stated otherwise)
- *   - Every data pointer is a DEVICE pointer on the current CUDA device, caller-owned, 16-byte
- *     aligned, fp32 (int32 for indices / counters).  The *_host entry points at the end take HOST
- *     pointers instead and say so.
+ *   - Every data pointer is a DEVICE pointer on the current CUDA device, caller-owned, fp32 (int32
+ *     for indices / counters).  The dictionary and the batched Y, X, R must be 16-byte aligned;
+ *     the vectors y, x, r of mp_recover need only their natural 4-byte alignment.  The *_host
+ *     entry points at the end take HOST pointers instead and say so.
  *   - The dictionary is ATOM-MAJOR: psi_t[m*ld + n] = Psi[n][m], m = 0..M-1 (atom / column of Psi),
  *     n = 0..N-1, ld >= N and ld % 4 == 0.  (= Psi^T row-major = Psi column-major; each atom is
  *     contiguous so the reduction over n is coalesced.)  Elements psi_t[m*ld + n], N <= n < ld, may
@@ -27,7 +28,8 @@
  *     never synchronise the host (exception: the stream-loop fallback algorithm, see mp_set_int).
  *     All outputs, n_iter included, are device memory and valid once the stream has reached the
  *     end of the call.
- *   - The library allocates nothing on the hot path and keeps no per-problem state between calls;
+ *   - The library allocates nothing on the hot path and keeps no per-problem state between calls
+ *     (the optional dictionary handle at the end is the one exception, and says what it keeps);
  *     the caller provides `workspace` (>= mp_workspace_bytes(N, M, B) bytes, 256-byte aligned).
  *   - Errors: a status code is returned, nothing is printed, nothing throws.  Argument errors are
  *     detected before anything is enqueued and leave every output untouched.  mp_last_error()
@@ -205,8 +207,9 @@ MP_API mp_status mp_recover_signs_many(const uint32_t* bits, int N, int M, int64
  *   idx_trace / c_trace   nullable, [q*ldt + t] for t < n_iter[q], ldt >= max_iter
  * Problem q's result equals mp_recover on (dictionary q, Y[q]) under the same arithmetic contract.  One thread-block
  * cluster (1-16 CTAs) owns a problem at a time: its dictionary is held in the cluster's shared memory for the whole solve
- * when it fits (<= ~3.5 MB), else streamed from L2; the argmax is exchanged through distributed shared memory with one
- * hardware cluster barrier per iteration; clusters draw problems from a device counter.  N > 2048 falls back to one
+ * when it fits (<= ~3.5 MB), else streamed from L2; the argmax is exchanged without any barrier instruction: every warp's packed
+ * key is stored into every CTA of the cluster with st.async, which also counts on the destination's mbarrier, and a CTA waits on
+ * its own mbarrier until all keys have landed; clusters draw problems from a device counter.  N > 2048 falls back to one
  * single-signal solve after another.  Knobs: "many_cluster" (CTAs per problem, 0 = auto), "many_threads", "many_stat"
  * (2 = never stationary), "many_l2_mb" (MB of dictionaries the plan keeps in flight, 0 = auto = 64).  Workspace: mp_workspace_bytes_many(N, M, P). */
 MP_API size_t mp_workspace_bytes_many(int N, int M, int P);
@@ -220,6 +223,9 @@ MP_API mp_status mp_recover_many(const float* psi_t, int N, int M, int64_t ld, i
 MP_API const char* mp_last_error(void);
 
 /* Tuning / diagnostic knobs (process-wide, not part of the method).  Unknown name -> MP_ERR_INVALID_ARG.
+ * NOT thread-safe: the knobs are plain process-wide variables that every solve reads when it is called.  Set them before
+ * solves are issued and do not change them while another host thread is inside a library call; with the knobs left alone,
+ * solves may be issued from several host threads (each call keeps its state in its own arguments and workspace).
  *   "algo"          0 = auto (default: 4 if one cluster can hold the dictionary in shared memory -- 4NM <= ~3.4 MB, N <= 2048 --
  *                   else 3 if it fits, else 1, else 2), 4 = the cluster kernel of mp_recover_many with P = 1 (N <= 2048),
  *                   1 = persistent cooperative kernel fed by TMA bulk
@@ -259,6 +265,31 @@ MP_API mp_status mp_recover_host(const float* psi_t, int N, int M, int64_t ld, i
 MP_API mp_status mp_recover_batched_host(const float* psi_t, int N, int M, int64_t ld, int normalize,
                                   const float* Y, int64_t ldy, int B, float eps, int max_iter,
                                   float* X, float* R, int* n_iter);
+
+/* ---- dictionary handle ("the host to device dictionary transfer only takes place once, since all signals are
+ * encoded/decoded with the same dictionary"; SURVEY 8(b) allows an optional opaque handle) -------------------------------
+ * mp_dictionary_create puts ONE dictionary on the current device and keeps it there:
+ *   psi_on_host != 0   psi_t is a HOST pointer (M rows of N floats, row stride ld >= N, any alignment; pinned memory makes the
+ *                      copy faster).  The library allocates the device copy (row stride N rounded up to 4), uploads it in chunks and, if normalize != 0, normalises each chunk on the device (Eq. 4)
+ *                      while the next one is still in flight.  The host buffer is not modified and may be freed on return.
+ *   psi_on_host == 0   psi_t is a DEVICE pointer (16-byte aligned, ld % 4 == 0) that the handle BORROWS: the caller keeps it alive until
+ *                      mp_dictionary_destroy; with normalize != 0 it is normalised in place.
+ * The call synchronises (a one-off per dictionary).  The handle also owns an internal stream, the solver workspace and the
+ * small per-call device buffers of the *_host_h entry points, so a steady-state call moves only y up and x~, r, n_iter down.
+ * A handle is used by one host thread at a time.  mp_dictionary_info returns the shape and the DEVICE pointer of the
+ * dictionary (for the device-pointer entry points above); any output may be NULL.
+ * mp_recover_host_h / mp_recover_batched_host_h: as mp_recover_host / mp_recover_batched_host (HOST pointers, synchronous,
+ * same arithmetic, same bits) without the dictionary argument; Y rows need only ldy >= N.  Traces (nullable) as in
+ * mp_recover_batched_traced: [b*ldt + t], ldt >= max_iter; entries t >= n_iter[b] are unspecified. */
+typedef struct mp_dictionary mp_dictionary;
+MP_API mp_status mp_dictionary_create(const float* psi_t, int psi_on_host, int N, int M, int64_t ld, int normalize,
+                               mp_dictionary** out);
+MP_API mp_status mp_dictionary_destroy(mp_dictionary* handle);   /* NULL is allowed */
+MP_API mp_status mp_dictionary_info(const mp_dictionary* handle, int* N, int* M, int64_t* ld, const float** psi_t_device);
+MP_API mp_status mp_recover_host_h(mp_dictionary* handle, const float* y, float eps, int max_iter,
+                            float* x, float* r, int* n_iter, int* idx_trace, float* c_trace);
+MP_API mp_status mp_recover_batched_host_h(mp_dictionary* handle, const float* Y, int64_t ldy, int B, float eps, int max_iter,
+                                    float* X, float* R, int* n_iter, int* idx_trace, float* c_trace, int64_t ldt);
 
 #ifdef __cplusplus
 }

@@ -29,12 +29,16 @@ MP_OK, MP_ERR_INVALID_ARG, MP_ERR_CUDA, MP_ERR_UNSUPPORTED, MP_ERR_WORKSPACE = r
 
 
 def _load():
+    """build() is a no-op when the library is newer than every source it depends on, so a stale libmp_b200.so (git-ignored, but
+    shipped with the tree) is never loaded silently after an edit of csrc/."""
     path = _build.LIB
-    if not os.path.exists(path):
-        try:
-            _build.build()
-        except Exception as e:  # loud: no fallback implementation exists
+    try:
+        _build.build()
+    except Exception as e:  # loud: no fallback implementation exists
+        if not os.path.exists(path):
             raise ImportError(f"libmp_b200.so is missing and could not be built with nvcc: {e}") from e
+        import warnings
+        warnings.warn(f"libmp_b200.so could not be rebuilt ({e}); loading the existing library, which may be older than csrc/")
     return C.CDLL(path)
 
 
@@ -94,6 +98,16 @@ lib.mp_recover_host.restype = _i
 lib.mp_recover_host.argtypes = [_vp, _i, _i, _i64, _i, _vp, _f, _i, _vp, _vp, _vp, _vp, _vp]
 lib.mp_recover_batched_host.restype = _i
 lib.mp_recover_batched_host.argtypes = [_vp, _i, _i, _i64, _i, _vp, _i64, _i, _f, _i, _vp, _vp, _vp]
+lib.mp_dictionary_create.restype = _i
+lib.mp_dictionary_create.argtypes = [_vp, _i, _i, _i, _i64, _i, C.POINTER(_vp)]
+lib.mp_dictionary_destroy.restype = _i
+lib.mp_dictionary_destroy.argtypes = [_vp]
+lib.mp_dictionary_info.restype = _i
+lib.mp_dictionary_info.argtypes = [_vp, C.POINTER(_i), C.POINTER(_i), C.POINTER(_i64), C.POINTER(_vp)]
+lib.mp_recover_host_h.restype = _i
+lib.mp_recover_host_h.argtypes = [_vp, _vp, _f, _i, _vp, _vp, _vp, _vp, _vp]
+lib.mp_recover_batched_host_h.restype = _i
+lib.mp_recover_batched_host_h.argtypes = [_vp, _vp, _i64, _i, _f, _i, _vp, _vp, _vp, _vp, _vp, _i64]
 
 
 def _check(status: int):
@@ -463,6 +477,12 @@ def _host(t: torch.Tensor, dtype, what: str):
     return t.data_ptr()
 
 
+def _host_dict(t: torch.Tensor):
+    if t.is_cuda or t.dtype != torch.float32 or t.dim() != 2 or not (t.shape[1] == 1 or t.stride(1) == 1):
+        raise TypeError("psi_t must be a CPU float32 [M, N] tensor with unit stride along N")
+    return t.data_ptr()
+
+
 def mp_recover_host(psi_t: torch.Tensor, y: torch.Tensor, eps: float, max_iter: int, *, normalize: bool = False,
                     trace: bool = False, device: int = 0) -> Recovered:
     """HOST tensors in, HOST tensors out (copies, kernels and the final synchronise inside the C call)."""
@@ -473,7 +493,7 @@ def mp_recover_host(psi_t: torch.Tensor, y: torch.Tensor, eps: float, max_iter: 
     it = torch.empty(max(max_iter, 1), dtype=torch.int32) if trace else None
     ct = torch.empty(max(max_iter, 1), dtype=torch.float32) if trace else None
     with torch.cuda.device(device):
-        _check(lib.mp_recover_host(_host(psi_t, torch.float32, "psi_t"), N, M, psi_t.stride(0) if M > 1 else N,
+        _check(lib.mp_recover_host(_host_dict(psi_t), N, M, psi_t.stride(0) if M > 1 else N,
                                    int(normalize), _host(y, torch.float32, "y"), float(eps), int(max_iter),
                                    x.data_ptr(), r.data_ptr(), n_iter.data_ptr(),
                                    it.data_ptr() if trace else None, ct.data_ptr() if trace else None))
@@ -488,7 +508,75 @@ def mp_recover_batched_host(psi_t: torch.Tensor, Y: torch.Tensor, eps: float, ma
     R = torch.empty(B, N, dtype=torch.float32).pin_memory()
     n_iter = torch.zeros(B, dtype=torch.int32).pin_memory()
     with torch.cuda.device(device):
-        _check(lib.mp_recover_batched_host(_host(psi_t, torch.float32, "psi_t"), N, M, psi_t.stride(0) if M > 1 else N,
+        _check(lib.mp_recover_batched_host(_host_dict(psi_t), N, M, psi_t.stride(0) if M > 1 else N,
                                            int(normalize), _host(Y, torch.float32, "Y"), N, B, float(eps), int(max_iter),
                                            X.data_ptr(), R.data_ptr(), n_iter.data_ptr()))
     return Recovered(X, R, n_iter, None, None, None)
+
+
+@dataclasses.dataclass
+class Dictionary:
+    """An mp_dictionary handle (the dictionary goes to the device once).  `psi_t` is a torch view of the device copy
+    when the handle borrowed a device tensor (kept alive here), else None."""
+    ptr: int
+    N: int
+    M: int
+    ld: int
+    device: int
+    psi_ptr: int
+    psi_t: torch.Tensor | None = None
+
+
+def mp_dictionary_create(psi_t: torch.Tensor, *, normalize: bool = False) -> Dictionary:
+    """psi_t[M, N] float32 on the HOST (uploaded, optionally normalised on the device; the host tensor is untouched) or on the
+    DEVICE (borrowed; normalised in place if asked).  The handle lives on the current CUDA device / the tensor's device."""
+    if not (psi_t.dtype == torch.float32 and psi_t.dim() == 2 and (psi_t.shape[1] == 1 or psi_t.stride(1) == 1)):
+        raise TypeError("psi_t must be a float32 [M, N] tensor with unit stride along N (atom-major)")
+    M, N = psi_t.shape
+    ld = psi_t.stride(0) if M > 1 else max(psi_t.stride(0), N)
+    out = _vp(None)
+    dev = psi_t.device if psi_t.is_cuda else torch.device("cuda", torch.cuda.current_device())
+    with torch.cuda.device(dev):
+        if psi_t.is_cuda:
+            torch.cuda.current_stream().synchronize()            # the handle works on its own stream
+        _check(lib.mp_dictionary_create(psi_t.data_ptr(), 0 if psi_t.is_cuda else 1, N, M, ld, int(normalize), C.byref(out)))
+    p = _vp(None)
+    _check(lib.mp_dictionary_info(out, None, None, None, C.byref(p)))
+    return Dictionary(out.value, N, M, ld, dev.index if dev.index is not None else 0, p.value, psi_t if psi_t.is_cuda else None)
+
+
+def mp_dictionary_destroy(h: Dictionary) -> None:
+    if h.ptr:
+        _check(lib.mp_dictionary_destroy(h.ptr))
+        h.ptr = 0
+        h.psi_t = None
+
+
+def mp_recover_host_h(h: Dictionary, y: torch.Tensor, eps: float, max_iter: int, *, trace: bool = False) -> Recovered:
+    """mp_recover_host without the dictionary transfer: HOST y in, HOST x~, r, n_iter (and traces) out; synchronous."""
+    x = torch.empty(h.M, dtype=torch.float32).pin_memory()
+    r = torch.empty(h.N, dtype=torch.float32).pin_memory()
+    n_iter = torch.zeros(1, dtype=torch.int32).pin_memory()
+    it = torch.empty(max(max_iter, 1), dtype=torch.int32) if trace else None
+    ct = torch.empty(max(max_iter, 1), dtype=torch.float32) if trace else None
+    if y.numel() != h.N:
+        raise ValueError("y must have N elements")
+    _check(lib.mp_recover_host_h(h.ptr, _host(y, torch.float32, "y"), float(eps), int(max_iter), x.data_ptr(), r.data_ptr(),
+                                 n_iter.data_ptr(), it.data_ptr() if trace else None, ct.data_ptr() if trace else None))
+    return Recovered(x, r, n_iter, it, ct, None)
+
+
+def mp_recover_batched_host_h(h: Dictionary, Y: torch.Tensor, eps: float, max_iter: int, *, trace: bool = False) -> Recovered:
+    if Y.dim() != 2 or Y.shape[1] != h.N:
+        raise ValueError("Y must be [B, N]")
+    B = Y.shape[0]
+    X = torch.empty(B, h.M, dtype=torch.float32).pin_memory()
+    R = torch.empty(B, h.N, dtype=torch.float32).pin_memory()
+    n_iter = torch.zeros(B, dtype=torch.int32).pin_memory()
+    ldt = max(max_iter, 1)
+    it = torch.empty(B, ldt, dtype=torch.int32) if trace else None
+    ct = torch.empty(B, ldt, dtype=torch.float32) if trace else None
+    _check(lib.mp_recover_batched_host_h(h.ptr, _host(Y, torch.float32, "Y"), h.N, B, float(eps), int(max_iter),
+                                         X.data_ptr(), R.data_ptr(), n_iter.data_ptr(),
+                                         it.data_ptr() if trace else None, ct.data_ptr() if trace else None, ldt))
+    return Recovered(X, R, n_iter, it, ct, None)

@@ -14,7 +14,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmp_b200.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-         "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "--use_fast_math=false"]
+         "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden"]
 
 
 def sources():
@@ -30,7 +30,7 @@ def deps():
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in deps()):
         return LIB
-    flags = [f for f in FLAGS if not f.startswith("--use_fast_math")] + os.environ.get("MP_B200_EXTRA_NVCC_FLAGS", "").split()
+    flags = FLAGS + os.environ.get("MP_B200_EXTRA_NVCC_FLAGS", "").split()
     if verbose:
         flags += ["-Xptxas", "-v"]
     objs = []

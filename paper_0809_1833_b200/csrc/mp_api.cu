@@ -64,9 +64,10 @@ size_t workspace_layout(int N, int M, int B, void* base, Workspace* ws)
     const size_t o_x64 = take(sizeof(double) * (size_t)B * M);     // must directly follow ctrl (one memset covers both)
     const size_t o_r64 = take(sizeof(double) * (size_t)B * Nr);
     const size_t o_r32 = take(sizeof(float) * (size_t)B * Nr);
-    const size_t o_keys = take(sizeof(unsigned long long) * 3 * (size_t)(B > 1 && B < 64 ? 64 : B));
+    // the lock-step tensor-core kernel always works on 64 key slots and 128 operand rows, whatever B >= 1 is
+    const size_t o_keys = take(sizeof(unsigned long long) * 3 * (size_t)(B < 64 ? 64 : B));
     const size_t o_state = take(sizeof(int) * 4 * (size_t)B);
-    const size_t o_rs = B > 1 ? take(sizeof(float) * 128 * Nr) : off;
+    const size_t o_rs = take(sizeof(float) * 128 * Nr);
     if (ws) {
         ws->ctrl = reinterpret_cast<unsigned long long*>(b + o_ctrl);
         ws->x64 = reinterpret_cast<double*>(b + o_x64);
@@ -74,13 +75,14 @@ size_t workspace_layout(int N, int M, int B, void* base, Workspace* ws)
         ws->r32 = reinterpret_cast<float*>(b + o_r32);
         ws->keys = reinterpret_cast<unsigned long long*>(b + o_keys);
         ws->state = reinterpret_cast<int*>(b + o_state);
-        ws->rs = B > 1 ? reinterpret_cast<float*>(b + o_rs) : nullptr;
+        ws->rs = reinterpret_cast<float*>(b + o_rs);
         ws->bytes = off;
     }
     return off;
 }
 
 static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+static bool aligned4(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 3u) == 0; }
 
 static mp_status check_dictionary(const float* psi_t, int N, int M, int64_t ld)
 {
@@ -233,7 +235,7 @@ mp_status mp_recover(const float* psi_t, int N, int M, int64_t ld,
     mp_status st = check_dictionary(psi_t, N, M, ld);
     if (st != MP_OK) return st;
     if (!y || !x || !r || !n_iter) return fail(MP_ERR_INVALID_ARG, "y, x, r and n_iter must be non-null");
-    if (!aligned16(y) || !aligned16(x) || !aligned16(r)) return fail(MP_ERR_INVALID_ARG, "y, x, r must be 16-byte aligned");
+    if (!aligned4(y) || !aligned4(x) || !aligned4(r)) return fail(MP_ERR_INVALID_ARG, "y, x, r must be 4-byte aligned");
     if (max_iter < 0) return fail(MP_ERR_INVALID_ARG, "max_iter must be >= 0 (got %d)", max_iter);
     if (!(eps >= 0.0f)) return fail(MP_ERR_INVALID_ARG, "eps must be >= 0 and not NaN");
     const size_t need = mp_workspace_bytes(N, M, 1);

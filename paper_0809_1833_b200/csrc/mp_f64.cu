@@ -290,7 +290,8 @@ static bool f64_plan(int N, int M, const DeviceInfo& di, F64Plan* plan)
     if (n2 <= 32) { A = 16; UC = 1; }
     else if (n2 <= 64) { A = 8; UC = 2; }
     else if (n2 <= 128) { A = 4; UC = 4; }
-    const int G = di.sm_count > 0 ? di.sm_count : 1;
+    int G = di.sm_count > 0 ? di.sm_count : 1;
+    if (options().grid > 0 && options().grid < G) G = (int)options().grid;      // the knob: fewer CTAs, each with a larger share
     if (G > kF64Slots) return false;
     const int atoms_max = (M + G - 1) / G;
     const int n_chunks = (n2 + 32 * UC - 1) / (32 * UC);
@@ -308,7 +309,7 @@ static bool f64_plan(int N, int M, const DeviceInfo& di, F64Plan* plan)
         }
     }
     plan->A = A; plan->UC = UC; plan->W = W; plan->smem = smem;
-    plan->grid = options().grid > 0 && options().grid < di.sm_count ? (int)options().grid : di.sm_count;
+    plan->grid = G;
     return true;
 }
 

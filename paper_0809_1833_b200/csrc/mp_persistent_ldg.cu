@@ -278,7 +278,8 @@ static bool ldg_plan(int N, int M, const DeviceInfo& di, LdgPlan* plan)
     if (n4 <= 32) { A = 16; UC = 1; }
     else if (n4 <= 64) { A = 8; UC = 2; }
     else if (n4 <= 128) { A = 4; UC = 4; }
-    const int G = di.sm_count > 0 ? di.sm_count : 1;
+    int G = di.sm_count > 0 ? di.sm_count : 1;
+    if (options().grid > 0 && options().grid < G) G = (int)options().grid;      // the knob: fewer CTAs, each with a larger share
     const int atoms_max = (M + G - 1) / G;
     const int n_chunks = (n4 + 32 * UC - 1) / (32 * UC);
     const int items = ((atoms_max + A - 1) / A) * n_chunks;
@@ -296,7 +297,7 @@ static bool ldg_plan(int N, int M, const DeviceInfo& di, LdgPlan* plan)
         }
     }
     plan->A = A; plan->UC = UC; plan->W = W; plan->smem = smem;
-    plan->grid = options().grid > 0 && options().grid < di.sm_count ? (int)options().grid : di.sm_count;
+    plan->grid = G;
     return true;
 }
 

@@ -19,6 +19,8 @@ C-contiguous, float32) -- the layout the C-ABI library takes (include/mp_b200.h)
 from __future__ import annotations
 
 import dataclasses
+import os
+
 import numpy as np
 
 _MASK = np.uint64(0xFFFFFFFFFFFFFFFF)
@@ -55,18 +57,33 @@ def standard_normal(seed: int, stream: int, index: np.ndarray) -> np.ndarray:
 
 # stream ids (arbitrary, fixed)
 _S_PSI, _S_SUPPORT, _S_VALUE, _S_SIGN = 1, 2, 3, 4
-_CHUNK_ROWS_BYTES = 64 << 20
+_CHUNK_ROWS_BYTES = 16 << 20
+
+
+def _for_row_blocks(N: int, M: int, fill) -> None:
+    """fill(m0, m1) over row blocks of the dictionary.  Every element is a function of (seed, stream, index) alone
+    (counter-based), so the blocks are independent and are filled by a few threads (numpy releases the GIL)."""
+    rows = max(1, _CHUNK_ROWS_BYTES // (8 * N))
+    blocks = [(m0, min(M, m0 + rows)) for m0 in range(0, M, rows)]
+    workers = min(len(blocks), os.cpu_count() or 1, 16)
+    if workers <= 1:
+        for b in blocks:
+            fill(*b)
+        return
+    from concurrent.futures import ThreadPoolExecutor
+    with ThreadPoolExecutor(workers) as ex:
+        list(ex.map(lambda b: fill(*b), blocks))
 
 
 def gaussian_dictionary(N: int, M: int, seed: int) -> np.ndarray:
     """psi_t[M, N] float32, entries i.i.d. N(0,1) (drawn in float64, rounded once).
     NOT normalised -- normalising columns (Eq. 4) is a step of the method."""
     out = np.empty((M, N), dtype=np.float32)
-    rows = max(1, _CHUNK_ROWS_BYTES // (8 * N))
-    for m0 in range(0, M, rows):
-        m1 = min(M, m0 + rows)
+
+    def fill(m0, m1):
         idx = np.arange(m0 * N, m1 * N, dtype=np.uint64)
         out[m0:m1] = standard_normal(seed, _S_PSI, idx).reshape(m1 - m0, N).astype(np.float32)
+    _for_row_blocks(N, M, fill)
     return out
 
 
@@ -76,12 +93,12 @@ def bernoulli_dictionary(N: int, M: int, seed: int) -> np.ndarray:
     power of 4, e.g. N=4096 -> 1/64)."""
     a = np.float32(1.0 / np.sqrt(float(N)))
     out = np.empty((M, N), dtype=np.float32)
-    rows = max(1, _CHUNK_ROWS_BYTES // (8 * N))
-    for m0 in range(0, M, rows):
-        m1 = min(M, m0 + rows)
+
+    def fill(m0, m1):
         idx = np.arange(m0 * N, m1 * N, dtype=np.uint64)
         bit = (hash_u64(seed, _S_PSI, idx) >> np.uint64(63)).astype(np.bool_)
         out[m0:m1] = np.where(bit, a, -a).reshape(m1 - m0, N)
+    _for_row_blocks(N, M, fill)
     return out
 
 

@@ -30,3 +30,37 @@ def pytest_collection_modifyitems(config, items):
     for it in items:
         if "gpu" in it.keywords:
             it.add_marker(skip)
+
+
+def pytest_terminal_summary(terminalreporter, exitstatus, config):
+    """How often the G1 state-drift allowance (reading R14b) was needed, and the worst observed errors of the session."""
+    try:
+        import grading
+    except Exception:
+        return
+    log = grading.LOG
+    if not log:
+        return
+    import json
+    used = [g for g in log if g["g1_allowance_used"]]
+    worst_c = max(log, key=lambda g: g["max_c_err"] / g["c_tol"])
+    summary = {
+        "grades": len(log),
+        "free_running_divergences": sum(1 for g in log if g["first_divergence"] >= 0),
+        "g1_allowance_used": len(used),
+        "g1_allowance_max": max((g["g1_allowance"] for g in used), default=0.0),
+        "g1_gap_max_when_used": max((g["g1_gap"] for g in used), default=0.0),
+        "max_c_err": max(g["max_c_err"] for g in log),
+        "max_c_err_over_tol": worst_c["max_c_err"] / worst_c["c_tol"],
+        "max_c_err_over_tol_shape": [worst_c["N"], worst_c["M"]],
+        "max_rnorm_rel_err": max(g["rnorm_rel_err"] for g in log),
+        "max_x_rel_err_vs_ref": max(g["x_rel_err_vs_ref"] for g in log),
+        "near_ties": sum(g["near_ties"] for g in log),
+        "legal_flips": sum(g["flips"] for g in log),
+        "iterations_graded": sum(g["n_iter_gpu"] for g in log),
+    }
+    terminalreporter.write_line("grading summary: " + json.dumps(summary))
+    out = os.path.join(ROOT, "gpurun_out")
+    if os.path.isdir(out):
+        with open(os.path.join(out, "grading_summary.json"), "w") as f:
+            json.dump({"summary": summary, "g1_allowance_cases": used}, f, indent=1)

@@ -3,8 +3,9 @@
 Implements the parity contract of BASELINE.json's north_star under the readings listed in DESIGN.md:
 
   G1 free-running: the GPU index sequence equals the oracle's up to the first iteration whose top-two
-     relative gap of |c| (on the oracle's own state) is <= 1e-4 plus the drift allowance 2 ||d|| / max|c|,
-     d = the difference of the two residuals accumulated from the step-value errors so far (each bounded by G3)
+     relative gap of |c| (on the oracle's own state) is <= 1e-4 plus the drift allowance
+     (|<d, psi_ref>| + |<d, psi_gpu>|) / max|c|, d = the difference of the two residuals accumulated from the
+     step-value errors so far (each bounded by G3); the Grade records whether and how much of it was used
      -- after a legal near-tie flip the two runs are different trajectories and cannot be compared step by step.
   G2 teacher-forced replay over the WHOLE GPU trace: the oracle is advanced with the GPU's own (index,
      step) pairs, so its state is the exact-arithmetic image of the GPU state; at every iteration the
@@ -37,6 +38,10 @@ def c_tol_tensor_core(N: int) -> float:
 NORM_TOL = 1e-4     # north_star: final ||r|| within 1e-4 relative
 X_TOL = 1e-4        # north_star: ||x_gpu - x_ref|| / ||x_ref||
 
+# Every grade of the session, so that the use of the G1 allowance and the worst observed errors are visible
+# (tests/conftest.py prints the summary and writes it to gpurun_out/grading_summary.json when that folder exists).
+LOG: list[dict] = []
+
 
 @dataclasses.dataclass
 class Grade:
@@ -49,6 +54,9 @@ class Grade:
     rnorm_rel_err: float
     x_rel_err_vs_ref: float
     exact_recovery: bool
+    g1_allowance_used: bool = False    # the free-running sequences diverged at an oracle gap ABOVE GAP_TOL, accepted by R14b
+    g1_allowance: float = 0.0          # 2 ||d|| / max|c| at that divergence (0 if the sequences never diverged)
+    g1_gap: float = 0.0                # the oracle's top-two gap at that divergence
 
 
 def grade_single(psi32: np.ndarray, y32: np.ndarray, eps: float, max_iter: int,
@@ -74,6 +82,7 @@ def grade_single(psi32: np.ndarray, y32: np.ndarray, eps: float, max_iter: int,
     L = min(t_gpu, ref.n_iter)
     diff = np.nonzero(idx_gpu[:L] != ref.idx[:L])[0]
     first_div = int(diff[0]) if diff.size else -1
+    g1_used, g1_allow, g1_gap = False, 0.0, 0.0
     if first_div >= 0:
         # The oracle's gap is measured on the ORACLE's state; the GPU decided on ITS state.  Up to first_div both
         # took the same atoms, so the two residuals differ only by the accumulated step-value errors (each within
@@ -81,11 +90,20 @@ def grade_single(psi32: np.ndarray, y32: np.ndarray, eps: float, max_iter: int,
         # ||d|| (unit atoms), which moves the top-two comparison by at most 2 ||d|| / max|c|.  A divergence is legal
         # if the oracle's gap is within GAP_TOL plus that drift allowance; G2 below still requires the GPU's pick
         # to be the argmax (or a <= 1e-4 near-tie) of the exact-arithmetic image of its own state at EVERY step.
+        # The allowance is the EXACT shift of the two correlations involved, |<d, psi_ref>| + |<d, psi_gpu>| (not the bound
+        # 2 ||d||), so it is as small as the accumulated step errors allow.  No constant cap can be derived for it: late in a
+        # run ||r_t|| has fallen by 4-5 orders of magnitude while d carries the (tolerated, G3) step errors of the early,
+        # large iterations, so the two runs are then simply two different valid trajectories.  Its use and size are
+        # recorded in the Grade and summarised at the end of the session (tests/conftest.py).
         d = np.zeros(N)
         for s_ in range(first_div):
             d += (c_gpu[s_] - ref.c[s_]) * psi32[idx_gpu[s_]].astype(np.float64)
         cmax = abs(ref.c[first_div])
-        allowance = GAP_TOL + 2.0 * float(np.linalg.norm(d)) / max(cmax, np.finfo(np.float64).tiny)
+        shift = abs(float(d @ psi32[ref.idx[first_div]].astype(np.float64))) + abs(float(d @ psi32[idx_gpu[first_div]].astype(np.float64)))
+        g1_allow = shift / max(cmax, np.finfo(np.float64).tiny)
+        g1_gap = float(ref.gap[first_div])
+        g1_used = g1_gap > GAP_TOL
+        allowance = GAP_TOL + g1_allow
         assert ref.gap[first_div] <= allowance, (
             f"free-running sequences diverge at t={first_div} where the oracle's top-two gap is {ref.gap[first_div]:.3e} "
             f"> {GAP_TOL} + state-drift allowance {allowance - GAP_TOL:.3e}")
@@ -141,8 +159,10 @@ def grade_single(psi32: np.ndarray, y32: np.ndarray, eps: float, max_iter: int,
             assert not np.any(np.abs(x_gpu[off]) > tau), "off-support coefficient above tau"
             big = [m for m in sup if abs(x_true[m]) >= 2 * tau]
             assert np.all(np.abs(x_gpu[big]) > tau), "a true coefficient is missing"
-    return Grade(t_gpu, ref.n_iter, first_div, int(np.sum(rp.gap <= GAP_TOL)), int(np.sum(~same)),
-                 max_c_err, rn_err, x_err_ref, exact)
+    g = Grade(t_gpu, ref.n_iter, first_div, int(np.sum(rp.gap <= GAP_TOL)), int(np.sum(~same)),
+              max_c_err, rn_err, x_err_ref, exact, g1_used, g1_allow, g1_gap)
+    LOG.append({"N": int(N), "M": int(M), "c_tol": float(c_tol), **dataclasses.asdict(g)})
+    return g
 
 
 def residual_at(psi32: np.ndarray, y32: np.ndarray, idx, c, t: int) -> np.ndarray:

@@ -128,3 +128,21 @@ def test_argument_errors_of_mp_recover_signs_many():
     assert call(ldy=32) == 1 and call(T=-1) == 1 and call(eps=float("nan")) == 1 and call(it=ok, ldt=2) == 1
     assert call(ws=None) == 4 and call(wsb=16) == 4
     assert lib.mp_workspace_bytes_signs_many(8, 8, 0) == 0 and lib.mp_workspace_bytes_signs_many(8, 8, 3) == 256
+
+
+def test_argument_errors_of_the_dictionary_handle():
+    """mp_dictionary_create / *_host_h validate on the host before any CUDA call; destroying NULL is allowed."""
+    from paper_0809_1833_b200.binding import lib
+    ok = C.c_void_p(4096)
+    out = C.c_void_p(None)
+    f = lib.mp_dictionary_create
+    assert f(None, 1, 8, 8, 8, 0, C.byref(out)) == 1 and out.value is None
+    assert f(ok, 1, 0, 8, 8, 0, C.byref(out)) == 1 and f(ok, 1, 8, 0, 8, 0, C.byref(out)) == 1
+    assert f(ok, 1, 8, 8, 6, 0, C.byref(out)) == 1 and f(ok, 0, 6, 8, 6, 0, C.byref(out)) == 1       # ld < N; device ld % 4
+    assert f(C.c_void_p(4100), 0, 8, 8, 8, 0, C.byref(out)) == 1                                     # misaligned device pointer
+    assert f(ok, 1, 8, 8, 8, 0, None) == 1
+    assert lib.mp_dictionary_destroy(None) == 0
+    assert lib.mp_dictionary_info(None, None, None, None, None) == 1
+    assert lib.mp_recover_host_h(None, ok, 0.1, 1, ok, ok, ok, None, None) == 1
+    assert lib.mp_recover_batched_host_h(None, ok, 8, 1, 0.1, 1, ok, ok, ok, None, None, 1) == 1
+    assert b"handle" in lib.mp_last_error()

@@ -1,0 +1,260 @@
+"""Full-size GPU parity: every configuration of BASELINE.json in the launch configuration bench.py times, graded against
+the CPU oracle at EVERY iteration wherever the oracle finishes in seconds, and on dense samples at the 1 GiB size.
+
+P:70-84 define Matching Pursuit iteration by iteration, so the contract (tests/grading.py, G1-G6) is applied to the whole
+run: free-running agreement with the oracle up to the first near-tie (G1), teacher-forced replay of every pick and every
+step value (G2, G3), final residual and coefficients (G4), the stop rule at every t (G5) and exact recovery (G6).
+
+  cfg3 (the headline, 256 MiB, L2 residency hints auto-on)        seeds 1-3, full grading; hints on / off bit-identical
+  cfg4_2048 ... cfg4_16384 (4 MiB ... 256 MiB)                    full grading; hints auto / off bit-identical
+  cfg4_32768 (1 GiB)                                              every 16th iteration rebuilt in float64 + final residual + support
+  cfg5 (B = 64, tensor-core lock-step kernel)                     all 64 signals, full grading
+  Orthogonal MP / double precision / sign-packed at cfg3 size     full grading; hints on / off bit-identical where they apply
+"""
+import functools
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_0809_1833_b200 import synth
+import grading
+import problems
+import test_gpu_f64 as tf64
+import test_gpu_omp as tomp
+import test_gpu_parity as tpar
+import test_gpu_signs as tsigns
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def mp():
+    import paper_0809_1833_b200 as m
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    yield m
+    for k in ("algo", "batched_algo", "l2_resident_mb", "omp_algo"):
+        m.mp_set_int(k, 0)
+
+
+@functools.lru_cache(maxsize=2)
+def problem(name, seed):
+    return problems.make_problem(synth.config(name), seed)
+
+
+def run_hints(mp, pb, hints_mb, algo=0):
+    """One single-signal solve with the L2 residency knob set (0 = auto, 1 = off)."""
+    c = pb.cfg
+    mp.mp_set_int("l2_resident_mb", hints_mb)
+    try:
+        return tpar.run_single(mp, pb.psi32, pb.Y[0], c.eps, c.max_iter, algo)
+    finally:
+        mp.mp_set_int("l2_resident_mb", 0)
+
+
+# ------------------------------------------------------------------------------------------ cfg3: the headline configuration
+@pytest.mark.parametrize("seed", [1, 2, 3])
+def test_cfg3_every_iteration_graded(mp, seed):
+    """BASELINE.json's metric configuration exactly as bench.py launches it (algo auto = the register-streaming persistent
+    kernel, residency hints auto-on for a 256 MiB dictionary): the oracle's free run and the teacher-forced replay of the
+    whole GPU trace, G1-G6 at every iteration."""
+    pb = problem("cfg3", seed)
+    c = pb.cfg
+    out = run_hints(mp, pb, 0)
+    assert mp.mp_get_int("info_algo") == 3
+    x, r, t, idx, cc = out
+    g = grading.grade_single(pb.psi32, pb.Y[0], c.eps, c.max_iter, x, r, t, idx, cc, x_true=pb.X[0], support=pb.S[0])
+    assert g.exact_recovery and 800 < g.n_iter_gpu < 2500
+    if seed == 1:                                                           # the hints change where bytes come from, not one bit of the result
+        off = run_hints(mp, pb, 1)
+        for a, b in zip(out, off):
+            assert np.array_equal(a, b)
+    print(f"cfg3 seed {seed}: n_iter {g.n_iter_gpu} (oracle {g.n_iter_ref}), first divergence {g.first_divergence}, near-ties {g.near_ties}, "
+          f"flips {g.flips}, max step error {g.max_c_err:.2e} ||r||, g1 allowance used {g.g1_allowance_used} ({g.g1_allowance:.1e})")
+
+
+# ------------------------------------------------------------------------------------------ cfg4: the size sweep
+@pytest.mark.parametrize("M", [2048, 4096, 8192, 16384])
+def test_cfg4_every_iteration_graded(mp, M):
+    """BASELINE.json configs[3] (echoing the paper's M sweep): Gaussian dictionary, N = M/4, K = N/16, exactly 4K
+    iterations (eps = 0).  Full grading; residency hints auto and off give identical bits."""
+    pb = problem(f"cfg4_{M}", 1)
+    c = pb.cfg
+    out = run_hints(mp, pb, 0)
+    x, r, t, idx, cc = out
+    assert t == c.max_iter == 4 * c.K
+    g = grading.grade_single(pb.psi32, pb.Y[0], c.eps, c.max_iter, x, r, t, idx, cc, x_true=pb.X[0], support=pb.S[0])
+    off = run_hints(mp, pb, 1)
+    for a, b in zip(out, off):
+        assert np.array_equal(a, b)
+    if M == 8192:                                                           # a 64 MiB dictionary with the hints FORCED on (32 MB pinned)
+        forced = run_hints(mp, pb, 32)
+        for a, b in zip(out, forced):
+            assert np.array_equal(a, b)
+
+
+def test_cfg4_32768_one_gib_dictionary(mp):
+    """The largest size (N = 8192, M = 32768: 2^28 elements, 1 GiB, hints auto-on): every 16th iteration plus the first and
+    last few are rebuilt in float64 from the GPU trace and the pick and step value checked against one oracle correlation
+    pass each (G2, G3); final residual (G4); coefficients; support; hints off gives identical bits."""
+    pb = problem("cfg4_32768", 1)
+    c = pb.cfg
+    out = run_hints(mp, pb, 0)
+    x, r, t, idx, cc = out
+    assert t == c.max_iter == 4 * c.K == 2048
+    ts = sorted(set(list(range(0, 4)) + list(range(4, t, 16)) + list(range(t - 4, t))))
+    res = grading.grade_sampled(pb.psi32, pb.Y[0], idx, cc, t, r, ts)
+    assert len(res) == len(ts)
+    assert set(idx.tolist()) <= set(pb.S[0].tolist())                       # N = 16K: never an off-support atom
+    coef = np.zeros(c.M); np.add.at(coef, idx, cc.astype(np.float64))
+    assert np.all(np.abs(x - coef) <= 6e-8 * np.abs(coef) + 1e-45)
+    off = run_hints(mp, pb, 1)
+    for a, b in zip(out, off):
+        assert np.array_equal(a, b)
+    print(f"cfg4_32768: {len(ts)} iterations checked, worst step error {max(e for _, _, e in res):.2e} ||r||")
+
+
+# ------------------------------------------------------------------------------------------ cfg5: batched, all 64 signals
+def test_cfg5_all_signals_every_iteration_graded(mp):
+    """CFG5 as bench.py launches it (batched_algo auto = the lock-step tensor-core kernel): ALL 64 signals get the full
+    teacher-forced grading (free run + replay of every iteration), not a sample."""
+    pb = problem("cfg5", 1)
+    c = pb.cfg
+    mp.mp_set_int("batched_algo", 0)
+    res = mp.mp_recover_batched(tpar.dev(pb.psi32), tpar.dev(pb.Y), c.eps, c.max_iter, trace=True)
+    torch.cuda.synchronize()
+    assert mp.mp_get_int("info_tc_clusters") > 0, "cfg5 must run on the tensor-core kernel"
+    X, R, T = res.x.cpu().numpy(), res.r.cpu().numpy(), res.n_iter.cpu().numpy()
+    I, Cc = res.idx_trace.cpu().numpy(), res.c_trace.cpu().numpy()
+    c_tol = grading.c_tol_tensor_core(c.N)
+    worst, used = 0.0, 0
+    for b in range(c.B):
+        t = int(T[b])
+        g = grading.grade_single(pb.psi32, pb.Y[b], c.eps, c.max_iter, X[b], R[b], t, I[b, :t], Cc[b, :t],
+                                 x_true=pb.X[b], support=pb.S[b], c_tol=c_tol)
+        assert g.exact_recovery and 300 < t < 1500
+        worst = max(worst, g.max_c_err); used += int(g.g1_allowance_used)
+    print(f"cfg5: 64 signals, {int(T.sum())} iterations graded, worst step error {worst:.2e} ||r|| (tolerance {c_tol:.2e}), "
+          f"g1 allowance used by {used} signals")
+
+
+@pytest.mark.parametrize("algo", [0, 1])
+@pytest.mark.parametrize("B", [1, 65, 130])
+def test_batched_group_loop_and_single_signal_batch(mp, B, algo):
+    """B = 1 (auto: a single-signal solve; batched_algo 1: the lock-step kernel with one useful row pair) and B > 64 (groups of
+    64 signals reusing the workspace in stream order): every signal graded like a single run."""
+    N, M, K = 256, 4096, 10
+    cfg = problems.custom_config(N, M, K, eps=1e-5, max_iter=8 * K, B=B)
+    pb = problems.make_problem(cfg, seed=12)
+    mp.mp_set_int("batched_algo", algo)
+    try:
+        res = mp.mp_recover_batched(tpar.dev(pb.psi32), tpar.dev(pb.Y), cfg.eps, cfg.max_iter, trace=True)
+        torch.cuda.synchronize()
+    finally:
+        mp.mp_set_int("batched_algo", 0)
+    X, R, T = res.x.cpu().numpy(), res.r.cpu().numpy(), res.n_iter.cpu().numpy()
+    I, Cc = res.idx_trace.cpu().numpy(), res.c_trace.cpu().numpy()
+    c_tol = grading.c_tol_tensor_core(N)
+    for b in range(B):
+        t = int(T[b])
+        grading.grade_single(pb.psi32, pb.Y[b], cfg.eps, cfg.max_iter, X[b], R[b], t, I[b, :t], Cc[b, :t],
+                             x_true=pb.X[b], support=pb.S[b], nthreads=4, c_tol=c_tol)
+
+
+# ------------------------------------------------------------------------------------------ the NEXT rows at the headline size
+@pytest.mark.parametrize("algo", tomp.OMP_ALGOS)
+def test_cfg3_size_omp(mp, algo):
+    """Orthogonal MP at cfg3 (256 MiB: the persistent kernel's residency-hint path engages): exactly the support in K steps,
+    every step graded by the replay; hints on / off bit-identical."""
+    pb = problem("cfg3", 1)
+    c = pb.cfg
+    T = 2 * c.K
+    x, r, t, idx = tomp.run(mp, pb.psi32, pb.Y[0], c.eps, T, algo=algo)
+    assert mp.mp_get_int("info_omp_algo") == algo
+    assert t == c.K and set(idx.tolist()) == set(pb.S[0].tolist())
+    tomp.grade_omp(pb.psi32, pb.Y[0], c.eps, T, x, r, t, idx, x_true=pb.X[0], support=pb.S[0])
+    mp.mp_set_int("l2_resident_mb", 1)
+    try:
+        off = tomp.run(mp, pb.psi32, pb.Y[0], c.eps, T, algo=algo)
+    finally:
+        mp.mp_set_int("l2_resident_mb", 0)
+    for a, b in zip((x, r, t, idx), off):
+        assert np.array_equal(a, b)
+
+
+def test_cfg3_size_f64(mp):
+    """The double-precision path at cfg3's shape (float64 Bernoulli dictionary, 512 MiB, hints auto-on): full grading against
+    the oracle's float64 instantiation; hints off bit-identical."""
+    psi, x_true, s, y = tf64.make_f64(4096, 16384, 256, 1, dictionary="bernoulli")
+    out = tf64.run(mp, psi, y, tf64.EPS, 32768)
+    x, r, t, idx, c = out
+    g = tf64.grade(psi, y, tf64.EPS, 32768, x, r, t, idx, c, x_true=x_true, support=s)
+    assert g.exact_recovery and g.first_divergence == -1 and g.n_iter_gpu == g.n_iter_ref
+    mp.mp_set_int("l2_resident_mb", 1)
+    try:
+        off = tf64.run(mp, psi, y, tf64.EPS, 32768)
+    finally:
+        mp.mp_set_int("l2_resident_mb", 0)
+    for a, b in zip(out, off):
+        assert np.array_equal(a, b)
+
+
+def test_cfg3_signs_every_iteration_graded(mp):
+    """cfg3 from 8 MiB of sign bits: the full grading of the fp32 path against the oracle on the expanded dictionary."""
+    pb = problem("cfg3", 1)
+    c = pb.cfg
+    (x, r, t, idx, cc), bits = tsigns.run(mp, pb.psi32, pb.Y[0], c.eps, c.max_iter)
+    g = grading.grade_single(pb.psi32, pb.Y[0], c.eps, c.max_iter, x, r, t, idx, cc, x_true=pb.X[0], support=pb.S[0])
+    assert g.exact_recovery
+
+
+# ------------------------------------------------------------------------------------------ knobs and fallbacks the advisor flagged
+@pytest.mark.parametrize("algo", [3, "f64"])
+def test_grid_knob_smaller_grid_is_graded(mp, algo):
+    """Knob "grid" (fewer CTAs, each with a larger share of the atoms): the plan must size shared memory for the share it
+    really gets.  Full grading at half the SM count and at 3 CTAs."""
+    sm = torch.cuda.get_device_properties(0).multi_processor_count
+    for grid in (sm // 2, 3):
+        mp.mp_set_int("grid", grid)
+        try:
+            if algo == 3:
+                cfg = problems.custom_config(512, 4099, 24, eps=1e-4, max_iter=100)
+                pb = problems.make_problem(cfg, seed=4)
+                out = tpar.run_single(mp, pb.psi32, pb.Y[0], cfg.eps, cfg.max_iter, 3)
+                grading.grade_single(pb.psi32, pb.Y[0], cfg.eps, cfg.max_iter, *out)
+            else:
+                psi, x_true, s, y = tf64.make_f64(512, 4099, 24, 4)
+                out = tf64.run(mp, psi, y, 1e-4, 100)
+                tf64.grade(psi, y, 1e-4, 100, *out)
+        finally:
+            mp.mp_set_int("grid", 0)
+
+
+def test_many_fallback_accepts_unaligned_rows(mp):
+    """mp_recover_many for N > 2048 runs one single-signal solve per problem on rows Y + q*ldy, X + q*M, R + q*N: with N and M
+    not multiples of 4 those rows are only 4-byte aligned, which the header allows (ldy >= N)."""
+    N, M, K, P = 2050, 161, 6, 3
+    cfg = problems.custom_config(N, M, K, eps=1e-4, max_iter=6 * K)
+    pbs = [problems.make_problem(cfg, seed=20 + q) for q in range(P)]
+    ld = (N + 3) // 4 * 4
+    psi = torch.zeros((P, M, ld), dtype=torch.float32, device="cuda")
+    for q in range(P):
+        psi[q, :, :N] = tpar.dev(pbs[q].psi32)
+    Y = tpar.dev(np.stack([pb.Y[0] for pb in pbs]))
+    res = mp.mp_recover_many(psi[:, :, :N], Y, cfg.eps, cfg.max_iter, trace=True)
+    torch.cuda.synchronize()
+    for q in range(P):
+        t = int(res.n_iter[q].item())
+        grading.grade_single(pbs[q].psi32, pbs[q].Y[0], cfg.eps, cfg.max_iter, res.x[q].cpu().numpy(), res.r[q].cpu().numpy(), t,
+                             res.idx_trace[q].cpu().numpy()[:t], res.c_trace[q].cpu().numpy()[:t])
+
+
+def test_correlate_batched_all_zero_signals(mp):
+    """mp_correlate_batched with Y = 0: no MP iteration runs, C must still be written (all zeros)."""
+    cfg = problems.custom_config(256, 1024, 4, B=3)
+    psi32 = problems.normalise_on_host(synth.make_dictionary(cfg, seed=3))
+    Cg = mp.mp_correlate_batched(tpar.dev(psi32), torch.zeros(3, 256, dtype=torch.float32, device="cuda"),
+                                 C_out=torch.full((3, 1024), 7.0, dtype=torch.float32, device="cuda"))
+    torch.cuda.synchronize()
+    assert not Cg.cpu().numpy().any()
