@@ -43,6 +43,7 @@ def pytest_terminal_summary(terminalreporter, exitstatus, config):
         return
     import json
     used = [g for g in log if g["g1_allowance_used"]]
+    nd_used = [g for g in log if g["n_iter_drift_used"]]
     worst_c = max(log, key=lambda g: g["max_c_err"] / g["c_tol"])
     summary = {
         "grades": len(log),
@@ -50,6 +51,8 @@ def pytest_terminal_summary(terminalreporter, exitstatus, config):
         "g1_allowance_used": len(used),
         "g1_allowance_max": max((g["g1_allowance"] for g in used), default=0.0),
         "g1_gap_max_when_used": max((g["g1_gap"] for g in used), default=0.0),
+        "n_iter_drift_used": len(nd_used),
+        "n_iter_drift_max_over_threshold": max((g["n_iter_drift"] for g in nd_used), default=0.0),
         "max_c_err": max(g["max_c_err"] for g in log),
         "max_c_err_over_tol": worst_c["max_c_err"] / worst_c["c_tol"],
         "max_c_err_over_tol_shape": [worst_c["N"], worst_c["M"]],
@@ -63,4 +66,4 @@ def pytest_terminal_summary(terminalreporter, exitstatus, config):
     out = os.path.join(ROOT, "gpurun_out")
     if os.path.isdir(out):
         with open(os.path.join(out, "grading_summary.json"), "w") as f:
-            json.dump({"summary": summary, "g1_allowance_cases": used}, f, indent=1)
+            json.dump({"summary": summary, "g1_allowance_cases": used, "n_iter_drift_cases": nd_used}, f, indent=1)
