@@ -23,6 +23,19 @@ namespace mp {
 
 constexpr int kLdgMaxWarps = 32;
 
+// Optional phase timeline (profiling builds only, -DMP_K1_TIMING): clock64 stamps of thread 0 of a few CTAs per iteration.
+#ifdef MP_K1_TIMING
+constexpr int kK1StampIters = 96, kK1StampCtas = 4, kK1StampSlots = 10;
+__device__ long long g_k1_stamps[kK1StampCtas][kK1StampIters][kK1StampSlots];
+#define K1_STAMP(slot)                                                                                          \
+    do {                                                                                                        \
+        if (tid == 0 && t < kK1StampIters && (blockIdx.x % 49) == 0 && blockIdx.x / 49 < kK1StampCtas)          \
+            g_k1_stamps[blockIdx.x / 49][t][slot] = clock64();                                                  \
+    } while (0)
+#else
+#define K1_STAMP(slot) do {} while (0)
+#endif
+
 struct LdgParams {
     const float* psi_t;
     const float* y;
@@ -132,6 +145,7 @@ mp_persistent_ldg_kernel(const LdgParams p)
     int t = 0;
     // ---- the loop: while ||r|| > eps ||y|| and t < T -----------------------------------------------------------
     while ((rr > thresh2) && (t < p.max_iter)) {
+        K1_STAMP(0);
         // ---------- Eq. 9: items = (group of A atoms, chunk of 32*UC float4), dealt round-robin to the warps --------------
         // One item is always in flight per warp: `v` was loaded before the previous iteration's barrier (or in the
         // prologue), so the stream does not drain while the CTAs meet and update the residual.
@@ -173,7 +187,9 @@ mp_persistent_ldg_kernel(const LdgParams p)
         it = warp;                                                             // the dictionary never changes: the first item of
         have = it < n_items;                                                   // the next iteration is requested ahead of the barrier
         if (have) load_item(it);
+        K1_STAMP(1);
         __syncthreads();
+        K1_STAMP(2);
         // ---------- Eq. 9 finished per atom (chunks added in ascending order), Eq. 16 packed argmax ----------------------
         unsigned long long best = 0ull;
         for (int a = tid; a < n_atoms; a += THREADS) {
@@ -185,8 +201,11 @@ mp_persistent_ldg_kernel(const LdgParams p)
         best = warp_max_redux(best);
 
         // ---------- block argmax -> grid argmax, ONE grid barrier -------------------------------------------------
+        // (red.max + red.release + acquire spin + key read: 4 L2 hops of ~650 cycles.  Tagged-slot exchanges without atomics
+        //  or fences were measured and are slower at 148 CTAs -- hot-line polling; profiles/k1_boundary_r02.md.)
         if (lane == 0) wkey[warp] = best;
         __syncthreads();
+        K1_STAMP(3);
         if (warp == 0) {
             unsigned long long k = lane < W ? wkey[lane] : 0ull;
             k = warp_max_redux(k);
@@ -194,12 +213,15 @@ mp_persistent_ldg_kernel(const LdgParams p)
                 unsigned long long* slot_key = p.ctrl + 1 + (t % 3);
                 if (k) red_max_u64(slot_key, k);
                 red_add_release_u64(p.ctrl, 1ull);
+                K1_STAMP(4);
                 const unsigned long long target = (unsigned long long)(t + 1) * (unsigned long long)G;
                 while (ld_acquire_u64(p.ctrl) < target) {}
+                K1_STAMP(5);
                 *skey = ld_relaxed_u64(slot_key);
             }
         }
         __syncthreads();
+        K1_STAMP(6);
         const unsigned long long key = *skey;
         const int i = key_index(key);
         const float c = key_value(key);
@@ -209,22 +231,34 @@ mp_persistent_ldg_kernel(const LdgParams p)
         {
             const float4* psi4 = reinterpret_cast<const float4*>(p.psi_t + (int64_t)i * p.ld);
             double s2 = 0.0;
-            for (int j = tid; j < n4; j += THREADS) {
-                const float4 q = __ldg(psi4 + j);
-                const int n = j << 2;
-                double v0 = r64[n] - cd * (double)q.x;
-                double v1 = r64[n + 1] - cd * (double)q.y;
-                double v2 = r64[n + 2] - cd * (double)q.z;
-                double v3 = r64[n + 3] - cd * (double)q.w;
-                if (n + 3 >= p.N) {                                             // keep the pad of r at zero
-                    if (n + 1 >= p.N) v1 = 0.0;
-                    if (n + 2 >= p.N) v2 = 0.0;
-                    v3 = 0.0;
+            for (int j0 = tid; j0 < n4; j0 += 4 * THREADS) {                    // four 16-byte loads of psi_i in flight per thread
+                float4 q4[4];
+#pragma unroll
+                for (int u = 0; u < 4; u++) {
+                    const int j = j0 + u * THREADS;
+                    q4[u] = j < n4 ? __ldg(psi4 + j) : make_float4(0.f, 0.f, 0.f, 0.f);
                 }
-                r64[n] = v0; r64[n + 1] = v1; r64[n + 2] = v2; r64[n + 3] = v3;
-                *reinterpret_cast<float4*>(r32 + n) = make_float4((float)v0, (float)v1, (float)v2, (float)v3);
-                s2 += v0 * v0; s2 += v1 * v1; s2 += v2 * v2; s2 += v3 * v3;
+#pragma unroll
+                for (int u = 0; u < 4; u++) {
+                    const int j = j0 + u * THREADS;
+                    if (j >= n4) break;
+                    const float4 q = q4[u];
+                    const int n = j << 2;
+                    double v0 = r64[n] - cd * (double)q.x;
+                    double v1 = r64[n + 1] - cd * (double)q.y;
+                    double v2 = r64[n + 2] - cd * (double)q.z;
+                    double v3 = r64[n + 3] - cd * (double)q.w;
+                    if (n + 3 >= p.N) {                                         // keep the pad of r at zero
+                        if (n + 1 >= p.N) v1 = 0.0;
+                        if (n + 2 >= p.N) v2 = 0.0;
+                        v3 = 0.0;
+                    }
+                    r64[n] = v0; r64[n + 1] = v1; r64[n + 2] = v2; r64[n + 3] = v3;
+                    *reinterpret_cast<float4*>(r32 + n) = make_float4((float)v0, (float)v1, (float)v2, (float)v3);
+                    s2 += v0 * v0; s2 += v1 * v1; s2 += v2 * v2; s2 += v3 * v3;
+                }
             }
+            K1_STAMP(7);
             s2 = warp_sum(s2);
             if (lane == 0) red[warp] = s2;
         }
@@ -242,6 +276,7 @@ mp_persistent_ldg_kernel(const LdgParams p)
             rr = (((q0.x + q0.y) + (q1.x + q1.y)) + ((q2.x + q2.y) + (q3.x + q3.y))) +
                  (((q4.x + q4.y) + (q5.x + q5.y)) + ((q6.x + q6.y) + (q7.x + q7.y)));
         }
+        K1_STAMP(8);
         t += 1;
     }
 
@@ -353,3 +388,11 @@ mp_status launch_recover_persistent_ldg(const RecoverArgs& a, const Workspace& w
 }
 
 }  // namespace mp
+
+#ifdef MP_K1_TIMING
+extern "C" __attribute__((visibility("default"))) int mp_debug_k1_stamps(long long* out, size_t bytes)
+{
+    if (bytes > sizeof(mp::g_k1_stamps)) bytes = sizeof(mp::g_k1_stamps);
+    return (int)cudaMemcpyFromSymbol(out, mp::g_k1_stamps, bytes);
+}
+#endif

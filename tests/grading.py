@@ -104,7 +104,7 @@ def grade_single(psi32: np.ndarray, y32: np.ndarray, eps: float, max_iter: int,
         shift = abs(float(d @ psi32[ref.idx[first_div]].astype(np.float64))) + abs(float(d @ psi32[idx_gpu[first_div]].astype(np.float64)))
         g1_allow = shift / max(cmax, np.finfo(np.float64).tiny)
         g1_gap = float(ref.gap[first_div])
-        g1_used = g1_gap > GAP_TOL
+        g1_used = bool(g1_gap > GAP_TOL)
         allowance = GAP_TOL + g1_allow
         assert ref.gap[first_div] <= allowance, (
             f"free-running sequences diverge at t={first_div} where the oracle's top-two gap is {ref.gap[first_div]:.3e} "
@@ -155,7 +155,7 @@ def grade_single(psi32: np.ndarray, y32: np.ndarray, eps: float, max_iter: int,
                 d += (c_gpu[s_] - ref.c[s_]) * psi32[idx_gpu[s_]].astype(np.float64)
             nd = float(np.linalg.norm(d))
             nd_rel = nd / thr if thr > 0 else 0.0
-            nd_used = abs(edge - thr) > NORM_TOL * thr
+            nd_used = bool(abs(edge - thr) > NORM_TOL * thr)
             assert abs(edge - thr) <= NORM_TOL * thr + nd, (
                 f"n_iter differs by one away from the stopping threshold: | ||r_ref|| - thr | = {abs(edge - thr):.3e}, "
                 f"NORM_TOL * thr = {NORM_TOL * thr:.3e}, state drift ||d|| = {nd:.3e}")

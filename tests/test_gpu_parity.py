@@ -370,7 +370,8 @@ def test_dictionary_handle_matches_the_other_entry_points_bit_for_bit(mp):
     raw_odd = torch.from_numpy(pb.psi_raw)                                     # host row stride 250: not a multiple of 4
     raw = torch.zeros(3000, 252); raw[:, :250] = raw_odd; raw = raw[:, :250]   # the same dictionary with a padded stride
     hh = mp.mp_dictionary_create(raw_odd, normalize=True)                      # host -> device (re-pitched), normalised there
-    psi_d = dev(pb.psi_raw); mp.mp_normalize_columns(psi_d); torch.cuda.synchronize()
+    psi_d = torch.zeros(3000, 252, device="cuda")[:, :250]; psi_d.copy_(raw_odd)   # device row stride 252 (the boundary wants ld % 4 == 0)
+    mp.mp_normalize_columns(psi_d); torch.cuda.synchronize()
     assert hh.N == 250 and hh.M == 3000 and hh.psi_ptr != 0
     hd = mp.mp_dictionary_create(psi_d)                                        # borrowed device tensor
     assert hd.psi_ptr == psi_d.data_ptr()
@@ -382,9 +383,10 @@ def test_dictionary_handle_matches_the_other_entry_points_bit_for_bit(mp):
             got = mp.mp_recover_host_h(h, y, 1e-5, 96, trace=True)
             assert int(got.n_iter.item()) == t and torch.equal(got.x, ref.x) and torch.equal(got.r, ref.r)
             assert torch.equal(got.idx_trace[:t], ref.idx_trace[:t]) and torch.equal(got.c_trace[:t], ref.c_trace[:t])
-    grading.grade_single(psi_d.cpu().numpy(), pb.Y[2], 1e-5, 96, got.x.numpy(), got.r.numpy(), t, got.idx_trace.numpy()[:t], got.c_trace.numpy()[:t])
+    grading.grade_single(psi_d.cpu().contiguous().numpy(), pb.Y[2], 1e-5, 96, got.x.numpy(), got.r.numpy(), t, got.idx_trace.numpy()[:t], got.c_trace.numpy()[:t])
     # batched through the handle == mp_recover_batched on device tensors
-    refb = mp.mp_recover_batched(psi_d, dev(pb.Y), 1e-5, 96, trace=True)
+    Y_d = torch.zeros(5, 252, device="cuda")[:, :250]; Y_d.copy_(torch.from_numpy(pb.Y))      # the boundary wants ldy % 4 == 0
+    refb = mp.mp_recover_batched(psi_d, Y_d, 1e-5, 96, trace=True)
     torch.cuda.synchronize()
     gotb = mp.mp_recover_batched_host_h(hh, torch.from_numpy(pb.Y), 1e-5, 96, trace=True)
     assert torch.equal(gotb.x, refb.x.cpu()) and torch.equal(gotb.r, refb.r.cpu()) and torch.equal(gotb.n_iter, refb.n_iter.cpu())
