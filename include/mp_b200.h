@@ -235,6 +235,9 @@ MP_API const char* mp_last_error(void);
  *   "l2_resident_mb" algo 3 (and the float64 / Orthogonal MP kernels): MB of dictionary rows loaded L2::evict_last so that they
  *                   stay in L2 across iterations (the rest is loaded evict_first); 0 = auto (68 MB for dictionaries above
  *                   110 MB), 1 = off, other = that many MB for every dictionary larger than it
+ *   "balance"       algo 3, shares of >= 8 work items per warp (dictionaries that stream from HBM): 0 (default) = the warps of a CTA
+ *                   draw their work items from a counter, so a CTA finishes when its share is done and not when its slowest warp
+ *                   is (results do not depend on it), 1 = plain round-robin
  *   "l2_demote"     0 (default) = when a solve ends the pinned rows are handed back (applypriority L2::evict_normal), so later
  *                   kernels find a normal L2; 1 = left as they are (measurements)
  *   "warps"         consumer warps per CTA of the persistent kernel (0 = auto)

@@ -22,6 +22,7 @@ struct Options {
     int64_t algo = 0, warps = 0, slot_bytes = 0, depth = 0, grid = 0, chunk = 64;
     int64_t batched_algo = 0, batched_coop = 1;
     int64_t omp_algo = 0, info_omp_algo = 0;   // Orthogonal MP: 0 auto, 1 persistent kernel, 2 stream loop; and the one last used
+    int64_t balance = 0;               // register-streaming kernel: 0 = warps draw their items from a counter when the shares are long, 1 = plain round-robin
     int64_t l2_demote = 0;             // 0 = pinned rows are demoted to evict_normal when a solve ends, 1 = left pinned (measurements)
     int64_t l2_resident_mb = 0;        // register-streaming kernel: MB of dictionary kept in L2 with evict_last (0 = auto, 1 = off)
     int64_t many_cluster = 0, many_threads = 0, many_stat = 0, many_l2_mb = 0;   // cluster-per-problem kernel: CTAs per problem (0 auto), threads per CTA (0 auto), 2 = never stationary

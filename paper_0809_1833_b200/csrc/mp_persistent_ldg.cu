@@ -52,6 +52,7 @@ struct LdgParams {
     int max_iter;
     int demote;                 // hand the pinned rows back at the end (knob l2_demote, default on)
     int resident_groups;        // groups of A atoms per CTA loaded with L2::evict_last (0 = no residency hints)
+    int dynamic;                // long shares (the HBM-streaming regime): warps draw their work items from a counter (see the kernel)
 };
 
 __device__ __forceinline__ float4 ldg_cg4(const float4* p)
@@ -62,7 +63,8 @@ __device__ __forceinline__ float4 ldg_cg4(const float4* p)
 }
 
 // A atoms x UC float4 per lane: 16 independent 16-byte loads per lane per item.  (2, 8) for long rows, (16, 1) for short ones.
-template <int A, int UC>
+// DYN: the warps draw their work items from a shared-memory counter instead of taking every W-th one
+template <int A, int UC, bool DYN>
 __global__ void __launch_bounds__(512, 1)
 mp_persistent_ldg_kernel(const LdgParams p)
 {
@@ -76,9 +78,11 @@ mp_persistent_ldg_kernel(const LdgParams p)
     unsigned long long* wkey = reinterpret_cast<unsigned long long*>(r32 + p.Nr);
     double* red = reinterpret_cast<double*>(wkey + kLdgMaxWarps);
     unsigned long long* skey = reinterpret_cast<unsigned long long*>(red + kLdgMaxWarps);
+    int* next_item = reinterpret_cast<int*>(skey + 1);                          // items beyond the first W are drawn from this counter
     float* part = reinterpret_cast<float*>(skey + 2);                          // [atom of this CTA][chunk] partial dots
 
     if (tid < kLdgMaxWarps) red[tid] = 0.0;                                     // partial sums of absent warps stay 0
+    if (tid == 0) *next_item = THREADS >> 5;
     __syncthreads();
     const int a0 = (int)(((int64_t)blockIdx.x * p.M) / G);
     const int a1 = (int)(((int64_t)(blockIdx.x + 1) * p.M) / G);
@@ -146,10 +150,16 @@ mp_persistent_ldg_kernel(const LdgParams p)
     // ---- the loop: while ||r|| > eps ||y|| and t < T -----------------------------------------------------------
     while ((rr > thresh2) && (t < p.max_iter)) {
         K1_STAMP(0);
-        // ---------- Eq. 9: items = (group of A atoms, chunk of 32*UC float4), dealt round-robin to the warps --------------
+        // ---------- Eq. 9: items = (group of A atoms, chunk of 32*UC float4).  Warp w starts with item w; when the share is long
+        // (DYN: the HBM-streaming regime) every further item is drawn from a shared-memory counter: a warp whose rows came from L2
+        // (resident groups) or from a faster HBM channel takes more items, so the CTA is done when its share is done, not when its
+        // unluckiest warp is (profiles/k1_boundary_r02.md: the warps of one CTA finished up to 3 400 cycles apart).
+        // An atom's dot product is the same arithmetic whichever warp computes it, so the results do not depend on the dealing.
         // One item is always in flight per warp: `v` was loaded before the previous iteration's barrier (or in the
         // prologue), so the stream does not drain while the CTAs meet and update the residual.
         while (have) {
+            int nxt = it + W;                                                   // short shares (< 8 items per warp): plain round-robin
+            if (DYN && lane == 0) nxt = atomicAdd(next_item, 1);
             const int g = it / n_chunks, ch = it - g * n_chunks;
             const int atom0 = g * A;                                           // relative to a0
             const int jb = ch * 32 * UC + lane;
@@ -175,7 +185,7 @@ mp_persistent_ldg_kernel(const LdgParams p)
                     acc[a] = fmaf(v[a][u].z, rv.z, acc[a]); acc[a] = fmaf(v[a][u].w, rv.w, acc[a]);
                 }
             }
-            it += W;
+            it = DYN ? __shfl_sync(0xffffffffu, nxt, 0) : nxt;
             have = it < n_items;
             if (have) load_item(it);
 #pragma unroll
@@ -189,6 +199,7 @@ mp_persistent_ldg_kernel(const LdgParams p)
         if (have) load_item(it);
         K1_STAMP(1);
         __syncthreads();
+        if (DYN && tid == 0) *next_item = W;                                   // nobody draws again before the next barriers
         K1_STAMP(2);
         // ---------- Eq. 9 finished per atom (chunks added in ascending order), Eq. 16 packed argmax ----------------------
         unsigned long long best = 0ull;
@@ -231,32 +242,21 @@ mp_persistent_ldg_kernel(const LdgParams p)
         {
             const float4* psi4 = reinterpret_cast<const float4*>(p.psi_t + (int64_t)i * p.ld);
             double s2 = 0.0;
-            for (int j0 = tid; j0 < n4; j0 += 4 * THREADS) {                    // four 16-byte loads of psi_i in flight per thread
-                float4 q4[4];
-#pragma unroll
-                for (int u = 0; u < 4; u++) {
-                    const int j = j0 + u * THREADS;
-                    q4[u] = j < n4 ? __ldg(psi4 + j) : make_float4(0.f, 0.f, 0.f, 0.f);
+            for (int j = tid; j < n4; j += THREADS) {
+                const float4 q = __ldg(psi4 + j);
+                const int n = j << 2;
+                double v0 = r64[n] - cd * (double)q.x;
+                double v1 = r64[n + 1] - cd * (double)q.y;
+                double v2 = r64[n + 2] - cd * (double)q.z;
+                double v3 = r64[n + 3] - cd * (double)q.w;
+                if (n + 3 >= p.N) {                                             // keep the pad of r at zero
+                    if (n + 1 >= p.N) v1 = 0.0;
+                    if (n + 2 >= p.N) v2 = 0.0;
+                    v3 = 0.0;
                 }
-#pragma unroll
-                for (int u = 0; u < 4; u++) {
-                    const int j = j0 + u * THREADS;
-                    if (j >= n4) break;
-                    const float4 q = q4[u];
-                    const int n = j << 2;
-                    double v0 = r64[n] - cd * (double)q.x;
-                    double v1 = r64[n + 1] - cd * (double)q.y;
-                    double v2 = r64[n + 2] - cd * (double)q.z;
-                    double v3 = r64[n + 3] - cd * (double)q.w;
-                    if (n + 3 >= p.N) {                                         // keep the pad of r at zero
-                        if (n + 1 >= p.N) v1 = 0.0;
-                        if (n + 2 >= p.N) v2 = 0.0;
-                        v3 = 0.0;
-                    }
-                    r64[n] = v0; r64[n + 1] = v1; r64[n + 2] = v2; r64[n + 3] = v3;
-                    *reinterpret_cast<float4*>(r32 + n) = make_float4((float)v0, (float)v1, (float)v2, (float)v3);
-                    s2 += v0 * v0; s2 += v1 * v1; s2 += v2 * v2; s2 += v3 * v3;
-                }
+                r64[n] = v0; r64[n + 1] = v1; r64[n + 2] = v2; r64[n + 3] = v3;
+                *reinterpret_cast<float4*>(r32 + n) = make_float4((float)v0, (float)v1, (float)v2, (float)v3);
+                s2 += v0 * v0; s2 += v1 * v1; s2 += v2 * v2; s2 += v3 * v3;
             }
             K1_STAMP(7);
             s2 = warp_sum(s2);
@@ -302,7 +302,7 @@ mp_persistent_ldg_kernel(const LdgParams p)
 
 // ------------------------------------------------------------------------------------------------------------------
 struct LdgPlan {
-    int A, UC, W, grid;
+    int A, UC, W, grid, dynamic;
     size_t smem;
 };
 
@@ -321,10 +321,12 @@ static bool ldg_plan(int N, int M, const DeviceInfo& di, LdgPlan* plan)
     const size_t Nr = (size_t)round_up(N, 128);
     const size_t smem = Nr * 12 + 8 * (2 * kLdgMaxWarps + 4) + 4 * (size_t)atoms_max * n_chunks + 64;
     if (smem > (size_t)di.smem_optin) return false;
+    // long shares (>= 8 items per warp with 16 warps: the HBM-streaming regime): the warps draw items from a counter (knob "balance" = 1: off)
+    const bool dynamic = items >= 8 * 16 && options().balance != 1;
     // warps: the fullest rounds (see mp_persistent.cu make_plan); 8..16 warps, ties to more warps
     int W = 16;
     if (options().warps >= 1 && options().warps <= 16) W = (int)options().warps;
-    else {
+    else if (!dynamic) {                                                        // dynamic dealing needs no full rounds
         double best = -1.0;
         for (int w = 8; w <= 16; w++) {
             const double fill = (double)items / ((double)((items + w - 1) / w) * w);
@@ -332,7 +334,7 @@ static bool ldg_plan(int N, int M, const DeviceInfo& di, LdgPlan* plan)
         }
     }
     plan->A = A; plan->UC = UC; plan->W = W; plan->smem = smem;
-    plan->grid = G;
+    plan->grid = G; plan->dynamic = dynamic ? 1 : 0;
     return true;
 }
 
@@ -344,22 +346,27 @@ bool persistent_ldg_supported(int N, int M)
     return ldg_plan(N, M, di, &plan);
 }
 
-template <int A, int UC>
-static mp_status launch_ldg(const LdgParams& p, const LdgPlan& plan, int device, cudaStream_t stream)
+template <int A, int UC, bool DYN>
+static mp_status launch_ldg_mode(const LdgParams& p, const LdgPlan& plan, int device, cudaStream_t stream)
 {
     static thread_local int attr_dev = -1;
     if (attr_dev != device) {
-        MP_CUDA(cudaFuncSetAttribute(mp_persistent_ldg_kernel<A, UC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(227 * 1024)));
+        MP_CUDA(cudaFuncSetAttribute(mp_persistent_ldg_kernel<A, UC, DYN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(227 * 1024)));
         attr_dev = device;
     }
     int occ = 0;
-    MP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, mp_persistent_ldg_kernel<A, UC>, plan.W * 32, plan.smem));
+    MP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, mp_persistent_ldg_kernel<A, UC, DYN>, plan.W * 32, plan.smem));
     if (occ < 1) return fail(MP_ERR_UNSUPPORTED, "register-streaming persistent kernel does not fit one CTA per SM");
     void* args[] = {(void*)&p};
-    MP_CUDA(cudaLaunchCooperativeKernel((const void*)mp_persistent_ldg_kernel<A, UC>, dim3(plan.grid), dim3(plan.W * 32), args,
+    MP_CUDA(cudaLaunchCooperativeKernel((const void*)mp_persistent_ldg_kernel<A, UC, DYN>, dim3(plan.grid), dim3(plan.W * 32), args,
                                         plan.smem, stream));
     count_launch();
     return MP_OK;
+}
+template <int A, int UC>
+static mp_status launch_ldg(const LdgParams& p, const LdgPlan& plan, int device, cudaStream_t stream)
+{
+    return p.dynamic ? launch_ldg_mode<A, UC, true>(p, plan, device, stream) : launch_ldg_mode<A, UC, false>(p, plan, device, stream);
 }
 
 mp_status launch_recover_persistent_ldg(const RecoverArgs& a, const Workspace& ws, cudaStream_t stream)
@@ -381,6 +388,7 @@ mp_status launch_recover_persistent_ldg(const RecoverArgs& a, const Workspace& w
     // L2 residency: only for dictionaries that do not fit in L2 anyway.  Knob "l2_resident_mb": 0 = auto (68 MB), 1 = off.
     p.demote = options().l2_demote != 1;
     p.resident_groups = l2_resident_groups(4.0 * (double)a.ld * a.M, plan.grid, 4.0 * (double)a.ld * plan.A);
+    p.dynamic = plan.dynamic;
     if (plan.A == 16) return launch_ldg<16, 1>(p, plan, di.device, stream);
     if (plan.A == 8) return launch_ldg<8, 2>(p, plan, di.device, stream);
     if (plan.A == 4) return launch_ldg<4, 4>(p, plan, di.device, stream);
