@@ -149,6 +149,51 @@ __device__ __forceinline__ void red_add_f64(double* p, double v)
 }
 
 // ------------------------------------------------------------------------------------------------
+// The iteration boundary shared by the grid-wide fp32 kernels (mp_persistent_ldg.cu, mp_persistent.cu, mp_signs.cu):
+// block argmax -> grid argmax with ONE grid barrier (Eq. 9 / Eq. 16), and CTA 0's bookkeeping of the step (Eq. 10, traces).
+//   ctrl[0]     monotonic arrive counter (iteration t is complete at (t + 1) * gridDim.x)
+//   ctrl[1..3]  key slots rotating with t mod 3: slot t is filled by red.max before the arrive, read after the spin, and
+//               zeroed again by CTA 0 during iteration t + 1 (every CTA has read it by then), two iterations before its reuse
+// All threads of every CTA call grid_argmax with their warp's best key; every thread gets the same winning key back.
+// wkey: kMaxWarps shared slots, skey: one shared slot.  Four dependent L2 hops (max acknowledged by the release fence ->
+// arrive -> spin -> key read); cheaper schemes were measured and lost at 148 CTAs (profiles/k1_boundary_r02.md).
+// stamp_arrive / stamp_done (profiling builds): clock64 of thread 0 after the arrive and after the spin.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned long long grid_argmax(unsigned long long warp_best, unsigned long long* wkey, unsigned long long* skey,
+                                                          unsigned long long* ctrl, int t, long long* stamp_arrive = nullptr,
+                                                          long long* stamp_done = nullptr)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, W = blockDim.x >> 5;
+    if (lane == 0) wkey[warp] = warp_best;
+    __syncthreads();
+    if (warp == 0) {
+        unsigned long long k = lane < W ? wkey[lane] : 0ull;
+        k = warp_max_redux(k);
+        if (lane == 0) {
+            unsigned long long* slot_key = ctrl + 1 + (t % 3);
+            if (k) red_max_u64(slot_key, k);
+            red_add_release_u64(ctrl, 1ull);
+            if (stamp_arrive) *stamp_arrive = clock64();
+            const unsigned long long target = (unsigned long long)(t + 1) * (unsigned long long)gridDim.x;
+            while (ld_acquire_u64(ctrl) < target) {}
+            if (stamp_done) *stamp_done = clock64();
+            *skey = ld_relaxed_u64(slot_key);
+        }
+    }
+    __syncthreads();
+    return *skey;
+}
+// one thread of CTA 0 (not the thread every CTA's barrier waits for): x~_i += c in float64 (Eq. 10), the traces, and the key slot
+// of iteration t - 1 handed back
+__device__ __forceinline__ void record_step(double* x64, int* idx_trace, float* c_trace, unsigned long long* ctrl, int t, int i, float c)
+{
+    red_add_f64(x64 + i, (double)c);
+    if (idx_trace) idx_trace[t] = i;
+    if (c_trace) c_trace[t] = c;
+    st_relaxed_u64(ctrl + 1 + ((t + 2) % 3), 0ull);
+}
+
+// ------------------------------------------------------------------------------------------------
 // L2 residency control.  A dictionary larger than L2, streamed cyclically, gets no reuse at all (ncu: DRAM traffic = 4NM
 // per iteration, L2 hit rate 0.2 %).  Loading a FIXED subset of the rows with the evict_last priority and the rest with
 // evict_first keeps that subset in L2 across iterations, so only the rest comes from HBM every iteration.  Measured on

@@ -236,23 +236,8 @@ mp_persistent_kernel(const PersistentParams p)
             }
         }
 
-        // ---------- block argmax -> grid argmax, ONE grid barrier -------------------------------------------------
-        if (lane == 0) wkey[warp] = best;
-        __syncthreads();
-        if (warp == 0) {
-            unsigned long long k = lane < W ? wkey[lane] : 0ull;
-            k = warp_max(k);
-            if (lane == 0) {
-                unsigned long long* slot_key = p.ctrl + 1 + (t % 3);
-                if (k) red_max_u64(slot_key, k);
-                red_add_release_u64(p.ctrl, 1ull);
-                const unsigned long long target = (unsigned long long)(t + 1) * (unsigned long long)G;
-                while (ld_acquire_u64(p.ctrl) < target) {}
-                *skey = ld_relaxed_u64(slot_key);
-            }
-        }
-        __syncthreads();
-        const unsigned long long key = *skey;
+        // ---------- block argmax -> grid argmax, ONE grid barrier (mp_common.cuh) ---------------------------------------------
+        const unsigned long long key = grid_argmax(best, wkey, skey, p.ctrl, t);
         const int i = key_index(key);
         const float c = key_value(key);
         const double cd = (double)c;
@@ -282,10 +267,7 @@ mp_persistent_kernel(const PersistentParams p)
         }
         // ---------- Eq. 10, Eq. 12, traces: CTA 0 only ---------------------------------------------------------------
         if (blockIdx.x == 0 && tid == 0) {
-            red_add_f64(p.x64 + i, cd);
-            if (p.idx_trace) p.idx_trace[t] = i;
-            if (p.c_trace) p.c_trace[t] = c;
-            st_relaxed_u64(p.ctrl + 1 + ((t + 2) % 3), 0ull);                   // slot of iteration t-1: everyone has read it
+            record_step(p.x64, p.idx_trace, p.c_trace, p.ctrl, t, i, c);
         }
         __syncthreads();
         rr = warp_sum(lane < W ? red[lane] : 0.0);

@@ -211,29 +211,18 @@ mp_persistent_ldg_kernel(const LdgParams p)
         }
         best = warp_max_redux(best);
 
-        // ---------- block argmax -> grid argmax, ONE grid barrier -------------------------------------------------
-        // (red.max + red.release + acquire spin + key read: 4 L2 hops of ~650 cycles.  Tagged-slot exchanges without atomics
-        //  or fences were measured and are slower at 148 CTAs -- hot-line polling; profiles/k1_boundary_r02.md.)
-        if (lane == 0) wkey[warp] = best;
-        __syncthreads();
+        // ---------- block argmax -> grid argmax, ONE grid barrier (mp_common.cuh) ---------------------------------------------
         K1_STAMP(3);
-        if (warp == 0) {
-            unsigned long long k = lane < W ? wkey[lane] : 0ull;
-            k = warp_max_redux(k);
-            if (lane == 0) {
-                unsigned long long* slot_key = p.ctrl + 1 + (t % 3);
-                if (k) red_max_u64(slot_key, k);
-                red_add_release_u64(p.ctrl, 1ull);
-                K1_STAMP(4);
-                const unsigned long long target = (unsigned long long)(t + 1) * (unsigned long long)G;
-                while (ld_acquire_u64(p.ctrl) < target) {}
-                K1_STAMP(5);
-                *skey = ld_relaxed_u64(slot_key);
-            }
+#ifdef MP_K1_TIMING
+        long long st_arrive = 0, st_done = 0;
+        const unsigned long long key = grid_argmax(best, wkey, skey, p.ctrl, t, &st_arrive, &st_done);
+        if (tid == 0 && t < kK1StampIters && (blockIdx.x % 49) == 0 && blockIdx.x / 49 < kK1StampCtas) {
+            g_k1_stamps[blockIdx.x / 49][t][4] = st_arrive; g_k1_stamps[blockIdx.x / 49][t][5] = st_done;
         }
-        __syncthreads();
+#else
+        const unsigned long long key = grid_argmax(best, wkey, skey, p.ctrl, t);
+#endif
         K1_STAMP(6);
-        const unsigned long long key = *skey;
         const int i = key_index(key);
         const float c = key_value(key);
         const double cd = (double)c;
@@ -264,10 +253,7 @@ mp_persistent_ldg_kernel(const LdgParams p)
         }
         // ---------- Eq. 10, Eq. 12, traces: CTA 0 only ---------------------------------------------------------------
         if (blockIdx.x == 0 && tid == THREADS - 32) {                          // not the thread every CTA's barrier waits for
-            red_add_f64(p.x64 + i, cd);
-            if (p.idx_trace) p.idx_trace[t] = i;
-            if (p.c_trace) p.c_trace[t] = c;
-            st_relaxed_u64(p.ctrl + 1 + ((t + 2) % 3), 0ull);                   // slot of iteration t-1: everyone has read it
+            record_step(p.x64, p.idx_trace, p.c_trace, p.ctrl, t, i, c);
         }
         __syncthreads();
         {                                                                       // W <= 16 partials (absent warps hold 0), fixed tree

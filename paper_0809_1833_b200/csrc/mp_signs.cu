@@ -150,22 +150,7 @@ mp_persistent_signs_kernel(const SignParams p)
             best = k > best ? k : best;
         }
         best = warp_max_redux(best);
-        if (lane == 0) wkey[warp] = best;
-        __syncthreads();
-        if (warp == 0) {
-            unsigned long long k = lane < W ? wkey[lane] : 0ull;
-            k = warp_max_redux(k);
-            if (lane == 0) {
-                unsigned long long* slot_key = p.ctrl + 1 + (t % 3);
-                if (k) red_max_u64(slot_key, k);
-                red_add_release_u64(p.ctrl, 1ull);
-                const unsigned long long target = (unsigned long long)(t + 1) * (unsigned long long)G;
-                while (ld_acquire_u64(p.ctrl) < target) {}
-                *skey = ld_relaxed_u64(slot_key);
-            }
-        }
-        __syncthreads();
-        const unsigned long long key = *skey;
+        const unsigned long long key = grid_argmax(best, wkey, skey, p.ctrl, t);        // block -> grid argmax, one grid barrier (mp_common.cuh)
         const int i = key_index(key);
         const float c = key_value(key);
         const double cd = (double)c;
@@ -186,10 +171,7 @@ mp_persistent_signs_kernel(const SignParams p)
             if (lane == 0) red[warp] = s2;
         }
         if (blockIdx.x == 0 && tid == THREADS - 32) {                          // not the thread every CTA's barrier waits for
-            red_add_f64(p.x64 + i, cd);
-            if (p.idx_trace) p.idx_trace[t] = i;
-            if (p.c_trace) p.c_trace[t] = c;
-            st_relaxed_u64(p.ctrl + 1 + ((t + 2) % 3), 0ull);
+            record_step(p.x64, p.idx_trace, p.c_trace, p.ctrl, t, i, c);
         }
         __syncthreads();
         rr = 0.0;
