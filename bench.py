@@ -242,11 +242,12 @@ class Workload:
         torch, mp = self.torch, self.mp
         stream = torch.cuda.current_stream()
         for attempt in range(2):
+            # the sampler runs from the warm-up on (the same load as the timed steps): a short timed region still gets samples
+            clocks = ClockSampler(gpu_index); clocks.start()
             for _ in range(warmup):
                 self.normalize(); self.solve()
             torch.cuda.synchronize()
             ev = [torch.cuda.Event(enable_timing=True) for _ in range(2 * steps + 2)]
-            clocks = ClockSampler(gpu_index); clocks.start()
             if dist: dist.barrier()
             torch.cuda.synchronize()
             l0 = mp.mp_launch_count()
