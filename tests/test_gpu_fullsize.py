@@ -115,6 +115,23 @@ def test_cfg4_32768_one_gib_dictionary(mp):
     print(f"cfg4_32768: {len(ts)} iterations checked, worst step error {max(e for _, _, e in res):.2e} ||r||")
 
 
+def test_item_dealing_does_not_change_results(mp):
+    """Long shares (cfg3: 224 work items per CTA): the warps draw their items from a shared-memory counter, so which warp computes
+    which atom differs from run to run.  An atom's dot product is the same arithmetic whichever warp computes it: two runs with the
+    counter and one with plain round-robin (knob balance = 1) must agree bit for bit, traces included."""
+    pb = problem("cfg3", 2)
+    a = run_hints(mp, pb, 0)
+    b = run_hints(mp, pb, 0)
+    mp.mp_set_int("balance", 1)
+    try:
+        c = run_hints(mp, pb, 0)
+    finally:
+        mp.mp_set_int("balance", 0)
+    assert a[2] > 800
+    for u, v, w in zip(a, b, c):
+        assert np.array_equal(u, v) and np.array_equal(u, w)
+
+
 # ------------------------------------------------------------------------------------------ cfg5: batched, all 64 signals
 def test_cfg5_all_signals_every_iteration_graded(mp):
     """CFG5 as bench.py launches it (batched_algo auto = the lock-step tensor-core kernel): ALL 64 signals get the full
