@@ -62,7 +62,8 @@ __device__ __forceinline__ void warp_best(double& c, int& idx)
     }
 }
 
-template <int A, int UC>
+// DYN (long shares, the HBM-streaming regime): warps draw their work items from a shared-memory counter, as in mp_persistent_ldg.cu
+template <int A, int UC, bool DYN>
 __global__ void __launch_bounds__(512, 1)
 mp_persistent_f64_kernel(const F64Params p)
 {
@@ -77,7 +78,8 @@ mp_persistent_f64_kernel(const F64Params p)
     double* wc = red + kF64MaxWarps;                                           // W   per-warp best c
     int* wi = reinterpret_cast<int*>(wc + kF64MaxWarps);                       // W   per-warp best index
     Cand* win = reinterpret_cast<Cand*>(wi + kF64MaxWarps);                    // 1   the winner of this iteration
-    double* part = reinterpret_cast<double*>(win + 1);                         // [atom of this CTA][chunk] partial dots
+    int* next_item = reinterpret_cast<int*>(win + 1);                          // DYN: items beyond the first W are drawn from this counter
+    double* part = reinterpret_cast<double*>(next_item + 2);                   // [atom of this CTA][chunk] partial dots
 
     const int a0 = (int)(((int64_t)blockIdx.x * p.M) / G);
     const int a1 = (int)(((int64_t)(blockIdx.x + 1) * p.M) / G);
@@ -138,11 +140,15 @@ mp_persistent_f64_kernel(const F64Params p)
     int it = warp;
     bool have = it < n_items;
     if (have) load_item(it);
+    if (DYN && tid == 0) *next_item = W;
+    __syncthreads();
     int t = 0;
     // ---- the loop: while ||r|| > eps ||y|| and t < T -----------------------------------------------------------
     while ((sqrt(rr) > thresh) && (t < p.max_iter)) {
-        // ---------- Eq. 9: items dealt round-robin to the warps, one always in flight -------------------------------------
+        // ---------- Eq. 9: items dealt round-robin to the warps (DYN: drawn from a counter), one always in flight -----------
         while (have) {
+            int nxt = it + W;
+            if (DYN && lane == 0) nxt = atomicAdd(next_item, 1);
             const int g = it / n_chunks, ch = it - g * n_chunks;
             const int atom0 = g * A;
             const int jb = ch * 32 * UC + lane;
@@ -163,7 +169,7 @@ mp_persistent_f64_kernel(const F64Params p)
                     acc[a] = fma(v[a][u].y, rv.y, acc[a]);
                 }
             }
-            it += W;
+            it = DYN ? __shfl_sync(0xffffffffu, nxt, 0) : nxt;
             have = it < n_items;
             if (have) load_item(it);
 #pragma unroll
@@ -176,6 +182,7 @@ mp_persistent_f64_kernel(const F64Params p)
         have = it < n_items;                                                   // next iteration requested ahead of the barrier
         if (have) load_item(it);
         __syncthreads();
+        if (DYN && tid == 0) *next_item = W;                                   // nobody draws again before the next barriers
         // ---------- Eq. 9 finished per atom (chunks in ascending order), Eq. 16 -------------------------------------------
         double bc = 0.0;
         int bi = kNoAtom;
@@ -279,7 +286,7 @@ normalize_columns_f64_kernel(double* __restrict__ psi_t, int N, int M, int64_t l
 
 // ------------------------------------------------------------------------------------------------------------------
 struct F64Plan {
-    int A, UC, W, grid;
+    int A, UC, W, grid; bool dynamic;
     size_t smem;
 };
 
@@ -310,24 +317,26 @@ static bool f64_plan(int N, int M, const DeviceInfo& di, F64Plan* plan)
     }
     plan->A = A; plan->UC = UC; plan->W = W; plan->smem = smem;
     plan->grid = G;
+    plan->dynamic = A == 2 && items >= 8 * 16 && options().balance != 1;         // long shares: see mp_persistent_ldg.cu
+    if (plan->dynamic && !(options().warps >= 1 && options().warps <= 16)) plan->W = 16;
     return true;
 }
 
 static size_t f64_workspace(int M) { return 256 + (sizeof(double) * (size_t)M + 255) / 256 * 256 + sizeof(Cand) * 2 * kF64Slots; }
 
-template <int A, int UC>
+template <int A, int UC, bool DYN = false>
 static mp_status launch_f64(const F64Params& p, const F64Plan& plan, int device, cudaStream_t stream)
 {
     static thread_local int attr_dev = -1;
     if (attr_dev != device) {
-        MP_CUDA(cudaFuncSetAttribute(mp_persistent_f64_kernel<A, UC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(227 * 1024)));
+        MP_CUDA(cudaFuncSetAttribute(mp_persistent_f64_kernel<A, UC, DYN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(227 * 1024)));
         attr_dev = device;
     }
     int occ = 0;
-    MP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, mp_persistent_f64_kernel<A, UC>, plan.W * 32, plan.smem));
+    MP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, mp_persistent_f64_kernel<A, UC, DYN>, plan.W * 32, plan.smem));
     if (occ < 1) return fail(MP_ERR_UNSUPPORTED, "float64 persistent kernel does not fit one CTA per SM");
     void* args[] = {(void*)&p};
-    MP_CUDA(cudaLaunchCooperativeKernel((const void*)mp_persistent_f64_kernel<A, UC>, dim3(plan.grid), dim3(plan.W * 32), args,
+    MP_CUDA(cudaLaunchCooperativeKernel((const void*)mp_persistent_f64_kernel<A, UC, DYN>, dim3(plan.grid), dim3(plan.W * 32), args,
                                         plan.smem, stream));
     count_launch();
     return MP_OK;
@@ -392,6 +401,7 @@ MP_API mp_status mp_recover_f64(const double* psi_t, int N, int M, int64_t ld,
     if (plan.A == 16) return launch_f64<16, 1>(p, plan, di.device, s);
     if (plan.A == 8) return launch_f64<8, 2>(p, plan, di.device, s);
     if (plan.A == 4) return launch_f64<4, 4>(p, plan, di.device, s);
+    if (plan.dynamic) return launch_f64<2, 8, true>(p, plan, di.device, s);
     return launch_f64<2, 8>(p, plan, di.device, s);
 }
 

@@ -42,7 +42,8 @@ __device__ __forceinline__ float4 omp_ldg_cg4(const float4* p)
     return v;
 }
 
-template <int A, int UC>
+// DYN (long shares, the HBM-streaming regime): warps draw their work items from a shared-memory counter, as in mp_persistent_ldg.cu
+template <int A, int UC, bool DYN>
 __global__ void __launch_bounds__(512, 1)
 mp_omp_persistent_kernel(const OmpPParams p)
 {
@@ -57,6 +58,7 @@ mp_omp_persistent_kernel(const OmpPParams p)
     unsigned long long* wkey = reinterpret_cast<unsigned long long*>(r32 + p.Nr);
     double* red = reinterpret_cast<double*>(wkey + kOmpPMaxWarps);             // 32
     unsigned long long* skey = reinterpret_cast<unsigned long long*>(red + kOmpPMaxWarps);
+    int* next_item = reinterpret_cast<int*>(skey + 1);                          // DYN: items beyond the first W are drawn from this counter
     double* wsl = reinterpret_cast<double*>(skey + 2);                         // SLp  slice of the direction being orthogonalised
     double* hbuf = wsl + p.SLp;                                                // Tld  reduced Q^T w of the current pass
     double* psum = hbuf + p.Tld;                                               // kOmpJGroups x SLp
@@ -182,11 +184,15 @@ mp_omp_persistent_kernel(const OmpPParams p)
     int it = warp;
     bool have = it < n_items;
     if (have) load_item(it);
+    if (DYN && tid == 0) *next_item = W;
+    __syncthreads();
     int t = 0;
     // ---- the loop: while ||r|| > eps ||y|| and t < T (the stop rule of MP) ------------------------------------------
     while ((sqrt(rr) > thresh) && (t < p.T)) {
-        // ---------- Eq. 9: items dealt round-robin to the warps, one always in flight ----------------------------------------
+        // ---------- Eq. 9: items dealt round-robin to the warps (DYN: drawn from a counter), one always in flight --------------
         while (have) {
+            int nxt = it + W;
+            if (DYN && lane == 0) nxt = atomicAdd(next_item, 1);
             const int g = it / n_chunks, ch = it - g * n_chunks;
             const int atom0 = g * A;
             const int jb = ch * 32 * UC + lane;
@@ -212,7 +218,7 @@ mp_omp_persistent_kernel(const OmpPParams p)
                     acc[a] = fmaf(v[a][u].z, rv.z, acc[a]); acc[a] = fmaf(v[a][u].w, rv.w, acc[a]);
                 }
             }
-            it += W;
+            it = DYN ? __shfl_sync(0xffffffffu, nxt, 0) : nxt;
             have = it < n_items;
             if (have) load_item(it);
 #pragma unroll
@@ -225,6 +231,7 @@ mp_omp_persistent_kernel(const OmpPParams p)
         have = it < n_items;
         if (have) load_item(it);                                               // next iteration's first item, ahead of the barriers
         __syncthreads();
+        if (DYN && tid == 0) *next_item = W;                                   // nobody draws again before the next barriers
         unsigned long long best = 0ull;
         for (int a = tid; a < n_atoms; a += THREADS) {
             float c = part[a * n_chunks];
@@ -343,6 +350,7 @@ mp_omp_persistent_kernel(const OmpPParams p)
 struct OmpPPlan {
     int A, UC, W, grid, SLp, atoms_max;
     size_t smem;
+    bool dynamic;
 };
 
 static bool omp_p_plan(int N, int M, int T, const DeviceInfo& di, OmpPPlan* plan)
@@ -370,6 +378,8 @@ static bool omp_p_plan(int N, int M, int T, const DeviceInfo& di, OmpPPlan* plan
         const double fill = (double)items / ((double)((items + w - 1) / w) * w);
         if (fill >= best) { best = fill; W = w; }
     }
+    plan->dynamic = A == 2 && items >= 8 * 16 && options().balance != 1;         // long shares: see mp_persistent_ldg.cu
+    if (plan->dynamic) W = 16;
     if (W * 32 < SL) W = (SL + 31) / 32;
     plan->A = A; plan->UC = UC; plan->W = W; plan->grid = G; plan->SLp = SLp; plan->atoms_max = atoms_max; plan->smem = smem;
     return true;
@@ -383,19 +393,19 @@ bool omp_persistent_supported(int N, int M, int T)
     return omp_p_plan(N, M, T, di, &plan);
 }
 
-template <int A, int UC>
+template <int A, int UC, bool DYN = false>
 static mp_status launch_omp_p(const OmpPParams& p, const OmpPPlan& plan, int device, cudaStream_t stream)
 {
     static thread_local int attr_dev = -1;
     if (attr_dev != device) {
-        MP_CUDA(cudaFuncSetAttribute(mp_omp_persistent_kernel<A, UC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(227 * 1024)));
+        MP_CUDA(cudaFuncSetAttribute(mp_omp_persistent_kernel<A, UC, DYN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(227 * 1024)));
         attr_dev = device;
     }
     int occ = 0;
-    MP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, mp_omp_persistent_kernel<A, UC>, plan.W * 32, plan.smem));
+    MP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, mp_omp_persistent_kernel<A, UC, DYN>, plan.W * 32, plan.smem));
     if (occ < 1) return fail(MP_ERR_UNSUPPORTED, "persistent Orthogonal MP kernel does not fit one CTA per SM");
     void* args[] = {(void*)&p};
-    MP_CUDA(cudaLaunchCooperativeKernel((const void*)mp_omp_persistent_kernel<A, UC>, dim3(plan.grid), dim3(plan.W * 32), args,
+    MP_CUDA(cudaLaunchCooperativeKernel((const void*)mp_omp_persistent_kernel<A, UC, DYN>, dim3(plan.grid), dim3(plan.W * 32), args,
                                         plan.smem, stream));
     count_launch();
     return MP_OK;
@@ -419,6 +429,7 @@ mp_status launch_omp_persistent(const OmpArgs& a, const OmpWs& ws, cudaStream_t 
     if (plan.A == 16) return launch_omp_p<16, 1>(p, plan, di.device, stream);
     if (plan.A == 8) return launch_omp_p<8, 2>(p, plan, di.device, stream);
     if (plan.A == 4) return launch_omp_p<4, 4>(p, plan, di.device, stream);
+    if (plan.dynamic) return launch_omp_p<2, 8, true>(p, plan, di.device, stream);
     return launch_omp_p<2, 8>(p, plan, di.device, stream);
 }
 
