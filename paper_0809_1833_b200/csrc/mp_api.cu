@@ -158,6 +158,7 @@ static int64_t* option_slot(const char* name)
     if (!strcmp(name, "l2_resident_mb")) return &o.l2_resident_mb;
     if (!strcmp(name, "l2_demote")) return &o.l2_demote;
     if (!strcmp(name, "balance")) return &o.balance;
+    if (!strcmp(name, "pingpong")) return &o.pingpong;
     if (!strcmp(name, "many_cluster")) return &o.many_cluster;
     if (!strcmp(name, "many_threads")) return &o.many_threads;
     if (!strcmp(name, "many_stat")) return &o.many_stat;

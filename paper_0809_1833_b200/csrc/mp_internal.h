@@ -22,6 +22,7 @@ struct Options {
     int64_t algo = 0, warps = 0, slot_bytes = 0, depth = 0, grid = 0, chunk = 64;
     int64_t batched_algo = 0, batched_coop = 1;
     int64_t omp_algo = 0, info_omp_algo = 0;   // Orthogonal MP: 0 auto, 1 persistent kernel, 2 stream loop; and the one last used
+    int64_t pingpong = 0;              // register-streaming kernel: reversed item order on odd iterations; 0 = auto (with the residency hints), 1 = off, 2 = on
     int64_t balance = 0;               // register-streaming kernel: 0 = warps draw their items from a counter when the shares are long, 1 = plain round-robin
     int64_t l2_demote = 0;             // 0 = pinned rows are demoted to evict_normal when a solve ends, 1 = left pinned (measurements)
     int64_t l2_resident_mb = 0;        // register-streaming kernel: MB of dictionary kept in L2 with evict_last (0 = auto, 1 = off)
@@ -57,11 +58,15 @@ static inline int round_up(int v, int m) { return (v + m - 1) / m * m; }
 // measured optimum on B200, for dictionaries above 110 MB -- up to ~100 MB the plain LRU behaviour of the L2 already serves a
 // cyclic stream (84 MB: 9.3 us per iteration without hints, 10.5 us with) and above it the stream thrashes (134 MB: 22.2 us
 // without, 15.2 us with).  1 = off; any other value = that many MB, for every dictionary larger than it.
-static inline int l2_resident_groups(double dict_bytes, int grid, double group_bytes)
+// auto_mb: 68 for a kernel that streams in the same order every iteration, 96 with the reversed order on odd iterations (K1's "ping-pong":
+// the pinned rows then share the L2 with a recency-served part of the stream, and the measured optimum moves up).
+// With it the recency-served part alone carries dictionaries up to ~140 MB (134 MB: 11.6 us per iteration without pinned rows, 12.8 with,
+// 15.3 for the same-order stream with 68 MB pinned), so the hints then start at auto_min_mb = 140.
+static inline int l2_resident_groups(double dict_bytes, int grid, double group_bytes, double auto_mb = 68.0, double auto_min_mb = 110.0)
 {
     const int64_t knob = options().l2_resident_mb;
-    const double target = knob == 0 ? 68e6 : knob == 1 ? 0.0 : 1e6 * (double)knob;
-    if (!(target > 0.0) || grid < 1 || !(dict_bytes > (knob == 0 ? 110e6 : target))) return 0;
+    const double target = knob == 0 ? 1e6 * auto_mb : knob == 1 ? 0.0 : 1e6 * (double)knob;
+    if (!(target > 0.0) || grid < 1 || !(dict_bytes > (knob == 0 ? 1e6 * auto_min_mb : target))) return 0;
     return (int)(target / grid / group_bytes);
 }
 

@@ -52,6 +52,7 @@ struct LdgParams {
     int max_iter;
     int demote;                 // hand the pinned rows back at the end (knob l2_demote, default on)
     int resident_groups;        // groups of A atoms per CTA loaded with L2::evict_last (0 = no residency hints)
+    int pingpong;               // dictionaries larger than L2: odd iterations visit the items in reverse order (see the kernel)
     int dynamic;                // long shares (the HBM-streaming regime): warps draw their work items from a counter (see the kernel)
 };
 
@@ -63,8 +64,12 @@ __device__ __forceinline__ float4 ldg_cg4(const float4* p)
 }
 
 // A atoms x UC float4 per lane: 16 independent 16-byte loads per lane per item.  (2, 8) for long rows, (16, 1) for short ones.
-// DYN: the warps draw their work items from a shared-memory counter instead of taking every W-th one
-template <int A, int UC, bool DYN>
+// DYN: the warps draw their work items from a shared-memory counter instead of taking every W-th one.
+// PP ("ping-pong"): odd iterations visit the CTA's items in reverse order.  A dictionary larger than L2, streamed in the same order every
+// iteration, gets no reuse out of an LRU cache; turned around at every iteration boundary, the rows read last are read first again, so whatever
+// part of L2 is not held by the pinned rows serves the first part of every pass (cfg3: 32.3 -> 28.7 us per iteration together with a larger pinned
+// set, profiles/k1_boundary_r02.md).  The order in which a CTA visits its items does not enter any result.
+template <int A, int UC, bool DYN, bool PP>
 __global__ void __launch_bounds__(512, 1)
 mp_persistent_ldg_kernel(const LdgParams p)
 {
@@ -112,7 +117,8 @@ mp_persistent_ldg_kernel(const LdgParams p)
     const float4* r4 = reinterpret_cast<const float4*>(r32);
     const uint64_t pol_last = l2_policy_evict_last(), pol_first = l2_policy_evict_first();
     float4 v[A][UC];
-    auto load_item = [&](int item) {
+    auto load_item = [&](int item, bool flip) {
+        if (flip) item = n_items - 1 - item;
         const int g = item / n_chunks, ch = item - g * n_chunks;
         const int jb = ch * 32 * UC + lane;
         if (A <= 4 && p.resident_groups > 0) {                                  // dictionary larger than L2: residency hints (long rows only:
@@ -145,7 +151,7 @@ mp_persistent_ldg_kernel(const LdgParams p)
     };
     int it = warp;
     bool have = it < n_items;
-    if (have) load_item(it);
+    if (have) load_item(it, false);
     int t = 0;
     // ---- the loop: while ||r|| > eps ||y|| and t < T -----------------------------------------------------------
     while ((rr > thresh2) && (t < p.max_iter)) {
@@ -160,7 +166,9 @@ mp_persistent_ldg_kernel(const LdgParams p)
         while (have) {
             int nxt = it + W;                                                   // short shares (< 8 items per warp): plain round-robin
             if (DYN && lane == 0) nxt = atomicAdd(next_item, 1);
-            const int g = it / n_chunks, ch = it - g * n_chunks;
+            const bool flip = PP && (t & 1);
+            const int itm = flip ? n_items - 1 - it : it;
+            const int g = itm / n_chunks, ch = itm - g * n_chunks;
             const int atom0 = g * A;                                           // relative to a0
             const int jb = ch * 32 * UC + lane;
             float acc[A];
@@ -187,7 +195,7 @@ mp_persistent_ldg_kernel(const LdgParams p)
             }
             it = DYN ? __shfl_sync(0xffffffffu, nxt, 0) : nxt;
             have = it < n_items;
-            if (have) load_item(it);
+            if (have) load_item(it, flip);
 #pragma unroll
             for (int a = 0; a < A; a++) {
                 const float c = warp_sum(acc[a]);
@@ -196,7 +204,7 @@ mp_persistent_ldg_kernel(const LdgParams p)
         }
         it = warp;                                                             // the dictionary never changes: the first item of
         have = it < n_items;                                                   // the next iteration is requested ahead of the barrier
-        if (have) load_item(it);
+        if (have) load_item(it, PP && ((t + 1) & 1));
         K1_STAMP(1);
         __syncthreads();
         if (DYN && tid == 0) *next_item = W;                                   // nobody draws again before the next barriers
@@ -332,19 +340,19 @@ bool persistent_ldg_supported(int N, int M)
     return ldg_plan(N, M, di, &plan);
 }
 
-template <int A, int UC, bool DYN>
+template <int A, int UC, bool DYN, bool PP>
 static mp_status launch_ldg_mode(const LdgParams& p, const LdgPlan& plan, int device, cudaStream_t stream)
 {
     static thread_local int attr_dev = -1;
     if (attr_dev != device) {
-        MP_CUDA(cudaFuncSetAttribute(mp_persistent_ldg_kernel<A, UC, DYN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(227 * 1024)));
+        MP_CUDA(cudaFuncSetAttribute(mp_persistent_ldg_kernel<A, UC, DYN, PP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(227 * 1024)));
         attr_dev = device;
     }
     int occ = 0;
-    MP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, mp_persistent_ldg_kernel<A, UC, DYN>, plan.W * 32, plan.smem));
+    MP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, mp_persistent_ldg_kernel<A, UC, DYN, PP>, plan.W * 32, plan.smem));
     if (occ < 1) return fail(MP_ERR_UNSUPPORTED, "register-streaming persistent kernel does not fit one CTA per SM");
     void* args[] = {(void*)&p};
-    MP_CUDA(cudaLaunchCooperativeKernel((const void*)mp_persistent_ldg_kernel<A, UC, DYN>, dim3(plan.grid), dim3(plan.W * 32), args,
+    MP_CUDA(cudaLaunchCooperativeKernel((const void*)mp_persistent_ldg_kernel<A, UC, DYN, PP>, dim3(plan.grid), dim3(plan.W * 32), args,
                                         plan.smem, stream));
     count_launch();
     return MP_OK;
@@ -352,7 +360,8 @@ static mp_status launch_ldg_mode(const LdgParams& p, const LdgPlan& plan, int de
 template <int A, int UC>
 static mp_status launch_ldg(const LdgParams& p, const LdgPlan& plan, int device, cudaStream_t stream)
 {
-    return p.dynamic ? launch_ldg_mode<A, UC, true>(p, plan, device, stream) : launch_ldg_mode<A, UC, false>(p, plan, device, stream);
+    if (p.dynamic) return p.pingpong ? launch_ldg_mode<A, UC, true, true>(p, plan, device, stream) : launch_ldg_mode<A, UC, true, false>(p, plan, device, stream);
+    return p.pingpong ? launch_ldg_mode<A, UC, false, true>(p, plan, device, stream) : launch_ldg_mode<A, UC, false, false>(p, plan, device, stream);
 }
 
 mp_status launch_recover_persistent_ldg(const RecoverArgs& a, const Workspace& ws, cudaStream_t stream)
@@ -373,7 +382,12 @@ mp_status launch_recover_persistent_ldg(const RecoverArgs& a, const Workspace& w
     p.eps = a.eps; p.max_iter = a.max_iter;
     // L2 residency: only for dictionaries that do not fit in L2 anyway.  Knob "l2_resident_mb": 0 = auto (68 MB), 1 = off.
     p.demote = options().l2_demote != 1;
-    p.resident_groups = l2_resident_groups(4.0 * (double)a.ld * a.M, plan.grid, 4.0 * (double)a.ld * plan.A);
+    // knob "pingpong": 0 = auto (dictionaries above 90 MB: below that the L2 serves the same-order stream by itself), 1 = off, 2 = on.
+    // Measured per size in profiles/k1_boundary_r02.md: reversed order alone up to 140 MB, reversed order + 96 MB of pinned rows above.
+    const double dict_bytes = 4.0 * (double)a.ld * a.M;
+    p.pingpong = options().pingpong == 2 || (options().pingpong == 0 && dict_bytes > 90e6);
+    p.resident_groups = p.pingpong ? l2_resident_groups(dict_bytes, plan.grid, 4.0 * (double)a.ld * plan.A, 96.0, 140.0)
+                                   : l2_resident_groups(dict_bytes, plan.grid, 4.0 * (double)a.ld * plan.A);
     p.dynamic = plan.dynamic;
     if (plan.A == 16) return launch_ldg<16, 1>(p, plan, di.device, stream);
     if (plan.A == 8) return launch_ldg<8, 2>(p, plan, di.device, stream);

@@ -115,7 +115,7 @@ def test_cfg4_32768_one_gib_dictionary(mp):
     print(f"cfg4_32768: {len(ts)} iterations checked, worst step error {max(e for _, _, e in res):.2e} ||r||")
 
 
-def test_item_dealing_does_not_change_results(mp):
+def test_item_dealing_and_visiting_order_do_not_change_results(mp):
     """Long shares (cfg3: 224 work items per CTA): the warps draw their items from a shared-memory counter, so which warp computes
     which atom differs from run to run.  An atom's dot product is the same arithmetic whichever warp computes it: two runs with the
     counter and one with plain round-robin (knob balance = 1) must agree bit for bit, traces included."""
@@ -127,9 +127,14 @@ def test_item_dealing_does_not_change_results(mp):
         c = run_hints(mp, pb, 0)
     finally:
         mp.mp_set_int("balance", 0)
+    mp.mp_set_int("pingpong", 1)                                               # same order every iteration (auto: reversed on odd ones)
+    try:
+        d = run_hints(mp, pb, 0)
+    finally:
+        mp.mp_set_int("pingpong", 0)
     assert a[2] > 800
-    for u, v, w in zip(a, b, c):
-        assert np.array_equal(u, v) and np.array_equal(u, w)
+    for u, v, w, z in zip(a, b, c, d):
+        assert np.array_equal(u, v) and np.array_equal(u, w) and np.array_equal(u, z)
 
 
 # ------------------------------------------------------------------------------------------ cfg5: batched, all 64 signals
