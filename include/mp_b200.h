@@ -237,8 +237,9 @@ MP_API const char* mp_last_error(void);
  *                   110 MB), 1 = off, other = that many MB for every dictionary larger than it
  *   "pingpong"      algo 3: odd iterations visit a CTA's work items in reverse order, so that the rows read last are read first again
  *                   and the part of the L2 not held by pinned rows serves the start of every pass (results do not depend on it);
- *                   0 = auto (dictionaries above 90 MB), 1 = off, 2 = on.  With it on, "l2_resident_mb" auto = 96 MB for
- *                   dictionaries above 140 MB (none below)
+ *                   0 = auto (dictionaries above 90 MB), 1 = off, 2 = on.  With it on, "l2_resident_mb" auto = 88 MB for
+ *                   dictionaries above 140 MB (none below), and "pin_margin_pct" (0 = auto = 10, 100 = none) percent of a CTA's
+ *                   rows at either end of its share are never pinned: the reversed order re-reads them soonest
  *   "balance"       algo 3, shares of >= 8 work items per warp (dictionaries that stream from HBM): 0 (default) = the warps of a CTA
  *                   draw their work items from a counter, so a CTA finishes when its share is done and not when its slowest warp
  *                   is (results do not depend on it), 1 = plain round-robin

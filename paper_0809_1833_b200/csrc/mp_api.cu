@@ -159,6 +159,7 @@ static int64_t* option_slot(const char* name)
     if (!strcmp(name, "l2_demote")) return &o.l2_demote;
     if (!strcmp(name, "balance")) return &o.balance;
     if (!strcmp(name, "pingpong")) return &o.pingpong;
+    if (!strcmp(name, "pin_margin_pct")) return &o.pin_margin_pct;
     if (!strcmp(name, "many_cluster")) return &o.many_cluster;
     if (!strcmp(name, "many_threads")) return &o.many_threads;
     if (!strcmp(name, "many_stat")) return &o.many_stat;

@@ -38,6 +38,7 @@ struct F64Params {
     int max_iter;
     int demote;                 // hand the pinned rows back at the end (knob l2_demote, default on)
     int resident_groups;        // groups of A atoms per CTA loaded L2::evict_last (mp_common.cuh), 0 = no hints
+    int pingpong, pin_margin;   // DYN kernels: reversed item order on odd iterations, unpinned groups at either end (mp_internal.h l2_plan)
 };
 
 __device__ __forceinline__ double2 ldg_cg_d2(const double2* p)
@@ -108,12 +109,17 @@ mp_persistent_f64_kernel(const F64Params p)
     const double2* r2 = reinterpret_cast<const double2*>(rres);
     double2 v[A][UC];
     const uint64_t pol_last = l2_policy_evict_last(), pol_first = l2_policy_evict_first();
-    auto load_item = [&](int item) {
+    auto group_is_pinned = [&](int g) {
+        const int e = DYN ? p.pin_margin : 0;
+        return g >= e && g < n_groups - e && l2_group_is_resident(g - e, p.resident_groups, n_groups - 2 * e);
+    };
+    auto load_item = [&](int item, bool flip) {
+        if (flip) item = n_items - 1 - item;
         const int g = item / n_chunks, ch = item - g * n_chunks;
         const int jb = ch * 32 * UC + lane;
         if (A <= 4 && p.resident_groups > 0) {                                  // dictionary larger than L2: residency hints (long rows only:
                                                                                 // the short-row variants have no registers to spare)
-            const uint64_t pol = l2_group_is_resident(g, p.resident_groups, n_groups) ? pol_last : pol_first;
+            const uint64_t pol = group_is_pinned(g) ? pol_last : pol_first;
 #pragma unroll
             for (int a = 0; a < A; a++) {
                 const int rel = g * A + a < n_atoms ? g * A + a : n_atoms - 1;
@@ -139,7 +145,7 @@ mp_persistent_f64_kernel(const F64Params p)
     };
     int it = warp;
     bool have = it < n_items;
-    if (have) load_item(it);
+    if (have) load_item(it, false);
     if (DYN && tid == 0) *next_item = W;
     __syncthreads();
     int t = 0;
@@ -149,7 +155,9 @@ mp_persistent_f64_kernel(const F64Params p)
         while (have) {
             int nxt = it + W;
             if (DYN && lane == 0) nxt = atomicAdd(next_item, 1);
-            const int g = it / n_chunks, ch = it - g * n_chunks;
+            const bool flip = DYN && p.pingpong && (t & 1);                    // odd iterations visit the items in reverse order (mp_persistent_ldg.cu)
+            const int itm = flip ? n_items - 1 - it : it;
+            const int g = itm / n_chunks, ch = itm - g * n_chunks;
             const int atom0 = g * A;
             const int jb = ch * 32 * UC + lane;
             double acc[A];
@@ -171,7 +179,7 @@ mp_persistent_f64_kernel(const F64Params p)
             }
             it = DYN ? __shfl_sync(0xffffffffu, nxt, 0) : nxt;
             have = it < n_items;
-            if (have) load_item(it);
+            if (have) load_item(it, flip);
 #pragma unroll
             for (int a = 0; a < A; a++) {
                 const double c = warp_sum(acc[a]);
@@ -180,7 +188,7 @@ mp_persistent_f64_kernel(const F64Params p)
         }
         it = warp;                                                             // the dictionary never changes: first item of the
         have = it < n_items;                                                   // next iteration requested ahead of the barrier
-        if (have) load_item(it);
+        if (have) load_item(it, DYN && p.pingpong && ((t + 1) & 1));
         __syncthreads();
         if (DYN && tid == 0) *next_item = W;                                   // nobody draws again before the next barriers
         // ---------- Eq. 9 finished per atom (chunks in ascending order), Eq. 16 -------------------------------------------
@@ -250,7 +258,7 @@ mp_persistent_f64_kernel(const F64Params p)
     // ---- hand the pinned rows back to the L2's normal replacement (see l2_demote_row) ------------------------------------------
     if (A <= 4 && p.resident_groups > 0 && p.demote) {
         for (int g = warp; g < n_groups; g += W) {
-            if (!l2_group_is_resident(g, p.resident_groups, n_groups)) continue;
+            if (!group_is_pinned(g)) continue;
             for (int a = 0; a < A; a++) {
                 const int rel = g * A + a < n_atoms ? g * A + a : n_atoms - 1;
                 l2_demote_row(p.psi_t + (int64_t)(a0 + rel) * p.ld, (size_t)p.Npad * 8, lane);
@@ -397,7 +405,8 @@ MP_API mp_status mp_recover_f64(const double* psi_t, int N, int M, int64_t ld,
     p.ld = ld; p.N = N; p.M = M; p.Npad = round_up(N, 2); p.Nr = round_up(N, 128);
     p.eps = eps; p.max_iter = max_iter;
     p.demote = options().l2_demote != 1;
-    p.resident_groups = l2_resident_groups(8.0 * (double)ld * M, plan.grid, 8.0 * (double)ld * plan.A);
+    const L2Plan l2 = l2_plan(8.0 * (double)ld * M, plan.grid, 8.0 * (double)ld * plan.A, ((M + plan.grid - 1) / plan.grid + plan.A - 1) / plan.A, plan.dynamic);
+    p.resident_groups = l2.resident_groups; p.pingpong = l2.pingpong; p.pin_margin = l2.pin_margin;
     if (plan.A == 16) return launch_f64<16, 1>(p, plan, di.device, s);
     if (plan.A == 8) return launch_f64<8, 2>(p, plan, di.device, s);
     if (plan.A == 4) return launch_f64<4, 4>(p, plan, di.device, s);

@@ -22,6 +22,7 @@ struct Options {
     int64_t algo = 0, warps = 0, slot_bytes = 0, depth = 0, grid = 0, chunk = 64;
     int64_t batched_algo = 0, batched_coop = 1;
     int64_t omp_algo = 0, info_omp_algo = 0;   // Orthogonal MP: 0 auto, 1 persistent kernel, 2 stream loop; and the one last used
+    int64_t pin_margin_pct = 0;        // with pingpong: percent of a CTA's groups at either end that are never pinned (0 = auto = 10, 100 = none)
     int64_t pingpong = 0;              // register-streaming kernel: reversed item order on odd iterations; 0 = auto (with the residency hints), 1 = off, 2 = on
     int64_t balance = 0;               // register-streaming kernel: 0 = warps draw their items from a counter when the shares are long, 1 = plain round-robin
     int64_t l2_demote = 0;             // 0 = pinned rows are demoted to evict_normal when a solve ends, 1 = left pinned (measurements)
@@ -58,7 +59,7 @@ static inline int round_up(int v, int m) { return (v + m - 1) / m * m; }
 // measured optimum on B200, for dictionaries above 110 MB -- up to ~100 MB the plain LRU behaviour of the L2 already serves a
 // cyclic stream (84 MB: 9.3 us per iteration without hints, 10.5 us with) and above it the stream thrashes (134 MB: 22.2 us
 // without, 15.2 us with).  1 = off; any other value = that many MB, for every dictionary larger than it.
-// auto_mb: 68 for a kernel that streams in the same order every iteration, 96 with the reversed order on odd iterations (K1's "ping-pong":
+// auto_mb: 68 for a kernel that streams in the same order every iteration, 88 with the reversed order on odd iterations (K1's "ping-pong":
 // the pinned rows then share the L2 with a recency-served part of the stream, and the measured optimum moves up).
 // With it the recency-served part alone carries dictionaries up to ~140 MB (134 MB: 11.6 us per iteration without pinned rows, 12.8 with,
 // 15.3 for the same-order stream with 68 MB pinned), so the hints then start at auto_min_mb = 140.
@@ -68,6 +69,26 @@ static inline int l2_resident_groups(double dict_bytes, int grid, double group_b
     const double target = knob == 0 ? 1e6 * auto_mb : knob == 1 ? 0.0 : 1e6 * (double)knob;
     if (!(target > 0.0) || grid < 1 || !(dict_bytes > (knob == 0 ? 1e6 * auto_min_mb : target))) return 0;
     return (int)(target / grid / group_bytes);
+}
+
+// The L2 plan of a register-streaming persistent kernel (K1, float64, Orthogonal MP) for one launch.
+//   pingpong         odd iterations visit a CTA's work items in reverse order (knob "pingpong": 0 = auto for dictionaries above 90 MB --
+//                    below that the L2 serves the same-order stream by itself --, 1 = off, 2 = on); only kernels that can do it ask for it
+//   resident_groups  groups of rows per CTA loaded evict_last: with the reversed order 88 MB for dictionaries above 140 MB (the
+//                    recency-served part alone carries smaller ones), without it 68 MB above 110 MB
+//   pin_margin       with the reversed order: groups at either end of a CTA's share that are never pinned (knob "pin_margin_pct", auto 10 %)
+// Measured per size in profiles/k1_boundary_r02.md.
+struct L2Plan { int pingpong, resident_groups, pin_margin; };
+static inline L2Plan l2_plan(double dict_bytes, int grid, double group_bytes, int groups_per_cta, bool can_pingpong)
+{
+    L2Plan l;
+    l.pingpong = can_pingpong && (options().pingpong == 2 || (options().pingpong == 0 && dict_bytes > 90e6));
+    l.resident_groups = l.pingpong ? l2_resident_groups(dict_bytes, grid, group_bytes, 88.0, 140.0) : l2_resident_groups(dict_bytes, grid, group_bytes);
+    const int64_t pct = options().pin_margin_pct == 0 ? 10 : options().pin_margin_pct >= 100 ? 0 : options().pin_margin_pct;
+    int e = l.pingpong ? (int)(pct * groups_per_cta / 100) : 0;
+    if (groups_per_cta - 2 * e < l.resident_groups + 1) e = (groups_per_cta - l.resident_groups - 1) / 2;
+    l.pin_margin = e > 0 ? e : 0;
+    return l;
 }
 
 // ---- launchers (each enqueues on `stream`, returns MP_OK or an error) ---------------------------------------

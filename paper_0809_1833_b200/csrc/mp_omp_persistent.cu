@@ -33,6 +33,7 @@ struct OmpPParams {
     float eps;
     int demote;                 // hand the pinned rows back at the end (knob l2_demote, default on)
     int resident_groups;        // groups of A atoms per CTA loaded L2::evict_last (mp_common.cuh), 0 = no hints
+    int pingpong, pin_margin;   // DYN kernels: reversed item order on odd iterations, unpinned groups at either end (mp_internal.h l2_plan)
 };
 
 __device__ __forceinline__ float4 omp_ldg_cg4(const float4* p)
@@ -108,12 +109,17 @@ mp_omp_persistent_kernel(const OmpPParams p)
     const float4* r4 = reinterpret_cast<const float4*>(r32);
     float4 v[A][UC];
     const uint64_t pol_last = l2_policy_evict_last(), pol_first = l2_policy_evict_first();
-    auto load_item = [&](int item) {
+    auto group_is_pinned = [&](int g) {
+        const int e = DYN ? p.pin_margin : 0;
+        return g >= e && g < n_groups - e && l2_group_is_resident(g - e, p.resident_groups, n_groups - 2 * e);
+    };
+    auto load_item = [&](int item, bool flip) {
+        if (flip) item = n_items - 1 - item;
         const int g = item / n_chunks, ch = item - g * n_chunks;
         const int jb = ch * 32 * UC + lane;
         if (A <= 4 && p.resident_groups > 0) {                                  // dictionary larger than L2: residency hints (long rows only:
                                                                                 // the short-row variants have no registers to spare)
-            const uint64_t pol = l2_group_is_resident(g, p.resident_groups, n_groups) ? pol_last : pol_first;
+            const uint64_t pol = group_is_pinned(g) ? pol_last : pol_first;
 #pragma unroll
             for (int a = 0; a < A; a++) {
                 const int rel = g * A + a < n_atoms ? g * A + a : n_atoms - 1;
@@ -183,7 +189,7 @@ mp_omp_persistent_kernel(const OmpPParams p)
 
     int it = warp;
     bool have = it < n_items;
-    if (have) load_item(it);
+    if (have) load_item(it, false);
     if (DYN && tid == 0) *next_item = W;
     __syncthreads();
     int t = 0;
@@ -193,7 +199,9 @@ mp_omp_persistent_kernel(const OmpPParams p)
         while (have) {
             int nxt = it + W;
             if (DYN && lane == 0) nxt = atomicAdd(next_item, 1);
-            const int g = it / n_chunks, ch = it - g * n_chunks;
+            const bool flip = DYN && p.pingpong && (t & 1);                    // odd iterations visit the items in reverse order (mp_persistent_ldg.cu)
+            const int itm = flip ? n_items - 1 - it : it;
+            const int g = itm / n_chunks, ch = itm - g * n_chunks;
             const int atom0 = g * A;
             const int jb = ch * 32 * UC + lane;
             float acc[A];
@@ -220,7 +228,7 @@ mp_omp_persistent_kernel(const OmpPParams p)
             }
             it = DYN ? __shfl_sync(0xffffffffu, nxt, 0) : nxt;
             have = it < n_items;
-            if (have) load_item(it);
+            if (have) load_item(it, flip);
 #pragma unroll
             for (int a = 0; a < A; a++) {
                 const float c = warp_sum(acc[a]);
@@ -229,7 +237,7 @@ mp_omp_persistent_kernel(const OmpPParams p)
         }
         it = warp;
         have = it < n_items;
-        if (have) load_item(it);                                               // next iteration's first item, ahead of the barriers
+        if (have) load_item(it, DYN && p.pingpong && ((t + 1) & 1));           // next iteration's first item, ahead of the barriers
         __syncthreads();
         if (DYN && tid == 0) *next_item = W;                                   // nobody draws again before the next barriers
         unsigned long long best = 0ull;
@@ -332,7 +340,7 @@ mp_omp_persistent_kernel(const OmpPParams p)
     // ---- hand the pinned rows back to the L2's normal replacement (see l2_demote_row) ------------------------------------------
     if (A <= 4 && p.resident_groups > 0 && p.demote) {
         for (int g = warp; g < n_groups; g += W) {
-            if (!l2_group_is_resident(g, p.resident_groups, n_groups)) continue;
+            if (!group_is_pinned(g)) continue;
             for (int a = 0; a < A; a++) {
                 const int rel = g * A + a < n_atoms ? g * A + a : n_atoms - 1;
                 l2_demote_row(p.psi_t + (int64_t)(a0 + rel) * p.ld, (size_t)p.Npad * 4, lane);
@@ -425,7 +433,8 @@ mp_status launch_omp_persistent(const OmpArgs& a, const OmpWs& ws, cudaStream_t 
     p.N = a.N; p.M = a.M; p.Npad = round_up(a.N, 4); p.Nr = round_up(a.N, 128); p.T = a.T; p.Tld = round_up(a.T, 32);
     p.SLp = plan.SLp; p.atoms_max = plan.atoms_max; p.eps = a.eps;
     p.demote = options().l2_demote != 1;
-    p.resident_groups = l2_resident_groups(4.0 * (double)a.ld * a.M, plan.grid, 4.0 * (double)a.ld * plan.A);
+    const L2Plan l2 = l2_plan(4.0 * (double)a.ld * a.M, plan.grid, 4.0 * (double)a.ld * plan.A, ((a.M + plan.grid - 1) / plan.grid + plan.A - 1) / plan.A, plan.dynamic);
+    p.resident_groups = l2.resident_groups; p.pingpong = l2.pingpong; p.pin_margin = l2.pin_margin;
     if (plan.A == 16) return launch_omp_p<16, 1>(p, plan, di.device, stream);
     if (plan.A == 8) return launch_omp_p<8, 2>(p, plan, di.device, stream);
     if (plan.A == 4) return launch_omp_p<4, 4>(p, plan, di.device, stream);

@@ -52,6 +52,7 @@ struct LdgParams {
     int max_iter;
     int demote;                 // hand the pinned rows back at the end (knob l2_demote, default on)
     int resident_groups;        // groups of A atoms per CTA loaded with L2::evict_last (0 = no residency hints)
+    int pin_margin;             // PP: groups at either end of a CTA's share that are never pinned
     int pingpong;               // dictionaries larger than L2: odd iterations visit the items in reverse order (see the kernel)
     int dynamic;                // long shares (the HBM-streaming regime): warps draw their work items from a counter (see the kernel)
 };
@@ -117,6 +118,12 @@ mp_persistent_ldg_kernel(const LdgParams p)
     const float4* r4 = reinterpret_cast<const float4*>(r32);
     const uint64_t pol_last = l2_policy_evict_last(), pol_first = l2_policy_evict_first();
     float4 v[A][UC];
+    // pinned groups: spread evenly over the share, or (PP) over its middle only -- the p.pin_margin groups at either end are the ones the
+    // reversed order re-reads soonest, they are served by recency and need no pin
+    auto group_is_pinned = [&](int g) {
+        const int e = PP ? p.pin_margin : 0;
+        return g >= e && g < n_groups - e && l2_group_is_resident(g - e, p.resident_groups, n_groups - 2 * e);
+    };
     auto load_item = [&](int item, bool flip) {
         if (flip) item = n_items - 1 - item;
         const int g = item / n_chunks, ch = item - g * n_chunks;
@@ -125,7 +132,7 @@ mp_persistent_ldg_kernel(const LdgParams p)
                                                                                 // the short-row variants have no registers to spare)
             // The resident groups are spread evenly over the CTA's share (Bresenham), so that L2 hits and HBM misses
             // interleave in time: with the resident rows first, HBM idled while every CTA read them (35.4 -> 33.3 us).
-            const uint64_t pol = l2_group_is_resident(g, p.resident_groups, n_groups) ? pol_last : pol_first;
+            const uint64_t pol = group_is_pinned(g) ? pol_last : pol_first;
 #pragma unroll
             for (int a = 0; a < A; a++) {
                 const int rel = g * A + a < n_atoms ? g * A + a : n_atoms - 1;
@@ -277,7 +284,7 @@ mp_persistent_ldg_kernel(const LdgParams p)
     // ---- hand the pinned rows back to the L2's normal replacement (see l2_demote_row) ------------------------------------------
     if (A <= 4 && p.resident_groups > 0 && p.demote) {
         for (int g = warp; g < n_groups; g += W) {
-            if (!l2_group_is_resident(g, p.resident_groups, n_groups)) continue;
+            if (!group_is_pinned(g)) continue;
             for (int a = 0; a < A; a++) {
                 const int rel = g * A + a < n_atoms ? g * A + a : n_atoms - 1;
                 l2_demote_row(p.psi_t + (int64_t)(a0 + rel) * p.ld, (size_t)p.Npad * 4, lane);
@@ -382,12 +389,9 @@ mp_status launch_recover_persistent_ldg(const RecoverArgs& a, const Workspace& w
     p.eps = a.eps; p.max_iter = a.max_iter;
     // L2 residency: only for dictionaries that do not fit in L2 anyway.  Knob "l2_resident_mb": 0 = auto (68 MB), 1 = off.
     p.demote = options().l2_demote != 1;
-    // knob "pingpong": 0 = auto (dictionaries above 90 MB: below that the L2 serves the same-order stream by itself), 1 = off, 2 = on.
-    // Measured per size in profiles/k1_boundary_r02.md: reversed order alone up to 140 MB, reversed order + 96 MB of pinned rows above.
-    const double dict_bytes = 4.0 * (double)a.ld * a.M;
-    p.pingpong = options().pingpong == 2 || (options().pingpong == 0 && dict_bytes > 90e6);
-    p.resident_groups = p.pingpong ? l2_resident_groups(dict_bytes, plan.grid, 4.0 * (double)a.ld * plan.A, 96.0, 140.0)
-                                   : l2_resident_groups(dict_bytes, plan.grid, 4.0 * (double)a.ld * plan.A);
+    const L2Plan l2 = l2_plan(4.0 * (double)a.ld * a.M, plan.grid, 4.0 * (double)a.ld * plan.A,
+                              ((a.M + plan.grid - 1) / plan.grid + plan.A - 1) / plan.A, true);
+    p.pingpong = l2.pingpong; p.resident_groups = l2.resident_groups; p.pin_margin = l2.pin_margin;
     p.dynamic = plan.dynamic;
     if (plan.A == 16) return launch_ldg<16, 1>(p, plan, di.device, stream);
     if (plan.A == 8) return launch_ldg<8, 2>(p, plan, di.device, stream);
