@@ -375,12 +375,13 @@ def main():
         per_it, per_it_off, tsrc = ncu_traffic(mp_kernel_name(mp, False))
     roofline = roofline_of(mp, cfg, m, per_it, tsrc)
     if per_it and "dram_frac" in roofline:
-        # frac can exceed 1: a fixed ~64 MB of the dictionary is kept in L2 across iterations (L2::evict_last loads), so
-        # the kernel moves fewer HBM bytes per iteration than the algorithmic 4NM.
-        roofline["note"] = ("frac = algorithmic bytes (4NM per iteration) / time against the HBM peak; it exceeds 1 because ~64 MB of "
-                            "the dictionary stay L2-resident by evict_last hints: ncu DRAM traffic is %.1f MB per iteration against "
-                            "%.1f MB algorithmic (profiles/persistent_r01.md); dram_frac is that traffic against the same peak; "
-                            "no_hint is the same launch with the hints switched off (every byte from HBM), timed in this run"
+        # frac can exceed 1: ~88 MB of the dictionary are pinned in L2 (L2::evict_last loads) and odd iterations visit the rows in
+        # reverse order, so that the rows read last are read first again: the kernel moves fewer HBM bytes per iteration than 4NM.
+        roofline["note"] = ("frac = algorithmic bytes (4NM per iteration) / time against the HBM peak; it exceeds 1 because part of the "
+                            "dictionary is served by L2 every iteration (88 MB of rows pinned by evict_last loads + the rows read last "
+                            "in one iteration are read first in the next): ncu DRAM traffic is %.1f MB per iteration against "
+                            "%.1f MB algorithmic (profiles/launches_r02.md); dram_frac is that traffic against the same peak; "
+                            "no_hint is the same launch with both switched off (every byte from HBM), timed in this run"
                             % (per_it / 1e6, (4.0 * N * M + 4.0 * N) / 1e6))
     if B > 1 and roofline["bound"] == "tensor":
         roofline["note"] = "see profiles/batched_r02.md for what limits the contraction and the per-iteration chain"
@@ -389,15 +390,15 @@ def main():
     extra = None
     default_run = args.config == "cfg3" and not args.knob and args.max_iter is None and world == 1 and not args.no_extra
     if default_run:
-        mp.mp_set_int("l2_resident_mb", 1)
+        mp.mp_set_int("l2_resident_mb", 1); mp.mp_set_int("pingpong", 1)
         try:
             mo = wl.timed(3, 3, local)
         finally:
-            mp.mp_set_int("l2_resident_mb", 0)
+            mp.mp_set_int("l2_resident_mb", 0); mp.mp_set_int("pingpong", 0)
         ro = roofline_of(mp, cfg, mo, per_it_off, tsrc)
         roofline["no_hint"] = {"us_per_iteration": ro["us_per_iteration"], "achieved": ro["achieved"], "frac": ro["frac"],
                                "dram_frac": ro.get("dram_frac"), "steps": 3, "warmup": 3, "clocks": mo["clocks"],
-                               "knob": "l2_resident_mb=1 (hints off): 4NM bytes per iteration come from HBM"}
+                               "knob": "l2_resident_mb=1 pingpong=1 (no pinned rows, same visiting order every iteration): all 4NM bytes per iteration come from HBM"}
 
     # ---- e2e: the host-buffer C-ABI call, H2D of the dictionary and y and D2H of x, r, n_iter inside the timed region ----
     e2e = None
