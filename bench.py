@@ -374,6 +374,10 @@ def main():
     if args.config == "cfg3" and not args.knob and args.max_iter is None and mp.mp_get_int("info_algo") == 3:
         per_it, per_it_off, tsrc = ncu_traffic(mp_kernel_name(mp, False))
     roofline = roofline_of(mp, cfg, m, per_it, tsrc)
+    if mp.mp_get_int("info_algo") == 3:
+        roofline["l2_plan"] = {"reversed_order_on_odd_iterations": bool(mp.mp_get_int("info_l2_pingpong")),
+                               "pinned_mb": int(mp.mp_get_int("info_l2_resident_mb")),
+                               "items_drawn_from_counter": bool(mp.mp_get_int("info_l2_dynamic"))}
     if per_it and "dram_frac" in roofline:
         # frac can exceed 1: ~88 MB of the dictionary are pinned in L2 (L2::evict_last loads) and odd iterations visit the rows in
         # reverse order, so that the rows read last are read first again: the kernel moves fewer HBM bytes per iteration than 4NM.

@@ -240,6 +240,7 @@ MP_API const char* mp_last_error(void);
  *                   0 = auto (dictionaries above 90 MB), 1 = off, 2 = on.  With it on, "l2_resident_mb" auto = 88 MB for
  *                   dictionaries above 140 MB (none below), and "pin_margin_pct" (0 = auto = 10, 100 = none) percent of a CTA's
  *                   rows at either end of its share are never pinned: the reversed order re-reads them soonest
+ *   "info_l2_pingpong", "info_l2_resident_mb", "info_l2_dynamic"  (read with mp_get_int) the L2 plan the last algo-3 launch used
  *   "balance"       algo 3, shares of >= 8 work items per warp (dictionaries that stream from HBM): 0 (default) = the warps of a CTA
  *                   draw their work items from a counter, so a CTA finishes when its share is done and not when its slowest warp
  *                   is (results do not depend on it), 1 = plain round-robin

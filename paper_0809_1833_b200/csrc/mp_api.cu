@@ -153,6 +153,9 @@ static int64_t* option_slot(const char* name)
     if (!strcmp(name, "batched_algo")) return &o.batched_algo;
     if (!strcmp(name, "batched_coop")) return &o.batched_coop;
     if (!strcmp(name, "info_algo")) return &o.info_algo;
+    if (!strcmp(name, "info_l2_pingpong")) return &o.info_l2_pingpong;
+    if (!strcmp(name, "info_l2_resident_mb")) return &o.info_l2_resident_mb;
+    if (!strcmp(name, "info_l2_dynamic")) return &o.info_l2_dynamic;
     if (!strcmp(name, "omp_algo")) return &o.omp_algo;
     if (!strcmp(name, "info_omp_algo")) return &o.info_omp_algo;
     if (!strcmp(name, "l2_resident_mb")) return &o.l2_resident_mb;

@@ -29,6 +29,7 @@ struct Options {
     int64_t l2_resident_mb = 0;        // register-streaming kernel: MB of dictionary kept in L2 with evict_last (0 = auto, 1 = off)
     int64_t many_cluster = 0, many_threads = 0, many_stat = 0, many_l2_mb = 0;   // cluster-per-problem kernel: CTAs per problem (0 auto), threads per CTA (0 auto), 2 = never stationary
     int64_t info_many_cluster = 0, info_many_stat = 0, info_many_clusters = 0, info_many_threads = 0;   // plan of its last launch
+    int64_t info_l2_pingpong = 0, info_l2_resident_mb = 0, info_l2_dynamic = 0;   // L2 plan of the last register-streaming launch (read-only use)
     int64_t info_algo = 0;             // kernel the last mp_recover call used (1, 2 or 3)
     int64_t info_tc_clusters = 0, info_tc_at = 0, info_tc_stages = 0;   // plan of the last batched tensor-core launch (read-only use)
 };

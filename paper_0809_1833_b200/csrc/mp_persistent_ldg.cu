@@ -393,6 +393,8 @@ mp_status launch_recover_persistent_ldg(const RecoverArgs& a, const Workspace& w
                               ((a.M + plan.grid - 1) / plan.grid + plan.A - 1) / plan.A, true);
     p.pingpong = l2.pingpong; p.resident_groups = l2.resident_groups; p.pin_margin = l2.pin_margin;
     p.dynamic = plan.dynamic;
+    options().info_l2_pingpong = p.pingpong; options().info_l2_dynamic = p.dynamic;
+    options().info_l2_resident_mb = (int64_t)((double)p.resident_groups * plan.grid * 4.0 * (double)a.ld * plan.A / 1e6 + 0.5);
     if (plan.A == 16) return launch_ldg<16, 1>(p, plan, di.device, stream);
     if (plan.A == 8) return launch_ldg<8, 2>(p, plan, di.device, stream);
     if (plan.A == 4) return launch_ldg<4, 4>(p, plan, di.device, stream);

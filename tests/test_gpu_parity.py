@@ -401,6 +401,28 @@ def test_dictionary_handle_matches_the_other_entry_points_bit_for_bit(mp):
     assert hh.ptr == 0
 
 
+def test_automatic_l2_plan_by_dictionary_size(mp):
+    """The plan the register-streaming kernel reports for itself (mp_internal.h l2_plan): same order and no pinned rows while the
+    dictionary fits the L2, reversed order alone for 90-140 MB, reversed order + 88 MB of pinned rows above; whatever the plan, the
+    outputs are the same bits as with everything switched off."""
+    for N, M, want_pp, want_mb in ((2048, 8192, 0, 0), (2048, 14336, 1, 0), (2048, 22528, 1, 88)):
+        g = torch.Generator(device="cuda"); g.manual_seed(N + M)
+        psi = torch.randn(M, N, device="cuda", generator=g); mp.mp_normalize_columns(psi)
+        y = torch.randn(N, device="cuda", generator=g)
+        mp.mp_set_int("algo", 3)
+        a = mp.mp_recover(psi, y, 0.0, 24, trace=True); torch.cuda.synchronize()
+        assert mp.mp_get_int("info_l2_pingpong") == want_pp
+        assert abs(mp.mp_get_int("info_l2_resident_mb") - want_mb) <= 6
+        mp.mp_set_int("pingpong", 1); mp.mp_set_int("l2_resident_mb", 1); mp.mp_set_int("balance", 1)
+        try:
+            b = mp.mp_recover(psi, y, 0.0, 24, trace=True); torch.cuda.synchronize()
+            assert mp.mp_get_int("info_l2_pingpong") == 0 and mp.mp_get_int("info_l2_resident_mb") == 0
+        finally:
+            mp.mp_set_int("pingpong", 0); mp.mp_set_int("l2_resident_mb", 0); mp.mp_set_int("balance", 0); mp.mp_set_int("algo", 0)
+        assert torch.equal(a.x, b.x) and torch.equal(a.r, b.r) and torch.equal(a.idx_trace, b.idx_trace) and torch.equal(a.c_trace, b.c_trace)
+        del psi
+
+
 # ------------------------------------------------------------------------------------------ the paper's row-major layout
 @pytest.mark.parametrize("aligned", [False, True])
 @pytest.mark.parametrize("N,M,ldr", [(256, 1024, None), (250, 333, 340), (1, 5, None), (4096, 300, None), (37, 1000, 1003), (65, 129, None),
