@@ -116,6 +116,41 @@ def test_ragged_shapes_full_grading(mp, N, M, K, ld, algo):
     grading.grade_single(pb.psi32, pb.Y[0], cfg.eps, cfg.max_iter, x, r, t, idx, cc)
 
 
+@pytest.mark.parametrize("f64", [False, True])
+@pytest.mark.parametrize("N,M,K,ld", RAGGED + [(64, 5000, 8, None), (200, 3000, 8, None), (500, 2000, 8, None), (1500, 40000, 12, None)])
+def test_forced_l2_plan_on_ragged_shapes(mp, N, M, K, ld, f64):
+    """The L2 mechanisms of the register-streaming kernels (reversed order on odd iterations, pinned rows kept off the ends of a share,
+    items drawn from a counter when the shares are long) only engage by themselves above 90 MB.  Here they are forced onto small ragged
+    shapes -- every (A, UC) variant, shares of 0, 1 and a few groups, a few pinned rows per share -- and must leave every output
+    bit unchanged against the run with all of them off; the forced run is graded in full."""
+    cfg = problems.custom_config(N, M, K, eps=1e-4, max_iter=6 * K + 3)
+    pb = problems.make_problem(cfg, seed=5)
+
+    def run():
+        if not f64:
+            return run_single(mp, pb.psi32, pb.Y[0], cfg.eps, cfg.max_iter, 3, ld)
+        ld2 = ((ld or N) + 1) // 2 * 2
+        psi = torch.zeros(M, ld2, dtype=torch.float64, device="cuda")[:, :N]; psi.copy_(torch.from_numpy(pb.psi32.astype(np.float64)))
+        res = mp.mp_recover_f64(psi, torch.from_numpy(pb.Y[0].astype(np.float64)).cuda(), cfg.eps, cfg.max_iter, trace=True)
+        torch.cuda.synchronize()
+        t = int(res.n_iter.item())
+        return (res.x.cpu().numpy(), res.r.cpu().numpy(), t, res.idx_trace.cpu().numpy()[:t], res.c_trace.cpu().numpy()[:t])
+
+    mp.mp_set_int("pingpong", 1); mp.mp_set_int("l2_resident_mb", 1); mp.mp_set_int("balance", 1)
+    try:
+        off = run()
+        for mb in (1, 2, 5):                                                     # no pinned rows / 2 MB / 5 MB of them (if the dictionary is larger)
+            mp.mp_set_int("pingpong", 2); mp.mp_set_int("l2_resident_mb", mb); mp.mp_set_int("balance", 0)
+            on = run()
+            for a, b in zip(off, on):
+                assert np.array_equal(a, b)
+    finally:
+        mp.mp_set_int("pingpong", 0); mp.mp_set_int("l2_resident_mb", 0); mp.mp_set_int("balance", 0)
+    if not f64:
+        x, r, t, idx, cc = on
+        grading.grade_single(pb.psi32, pb.Y[0], cfg.eps, cfg.max_iter, x, r, t, idx, cc)
+
+
 @pytest.mark.parametrize("N,M,K", [(20000, 64, 8), (16, 200000, 4), (19000, 160, 6), (3, 100000, 1)])
 def test_extreme_aspect_ratios_auto_dispatch(mp, N, M, K):
     """Shapes at the edges of the kernels' plans under algo = auto: a residual too long for shared memory (stream loop),
