@@ -95,6 +95,31 @@ MP_API mp_status mp_recover(const float* psi_t, int N, int M, int64_t ld,
                      int* idx_trace, float* c_trace,
                      void* workspace, size_t workspace_bytes, void* stream);
 
+/* mp_recover for callers that cannot provide a workspace because they cannot allocate device memory at all: a plug-in
+ * running inside a server or framework whose own pool already owns the whole GPU (cudaMalloc fails there, or the host's
+ * rules forbid it), or a latency-bound loop that must not risk the device-wide stall an allocation can cause.  Same loop
+ * (Eq. 8-12), same arguments minus the workspace, same arithmetic contract and -- for the same inputs -- the same
+ * bits as mp_recover run with knob "algo" = 3: it is that kernel (the persistent register-streaming one), with its scratch
+ * area (a 256-byte control block and the float64 accumulator of x~) placed in a fixed array inside the library image.
+ *   - No cudaMalloc / cudaFree / pool allocation, and no library routine that allocates, is called on any path of this
+ *     entry point.  The caller still owns and passes every input and output (device pointers, as for mp_recover).
+ *   - Limit: M <= MP_NOALLOC_MAX_M atoms; a larger M returns MP_ERR_UNSUPPORTED with a message and touches nothing.
+ *     Shapes the register-streaming kernel itself cannot take (N above roughly 18 000: the residual no longer fits in shared
+ *     memory) are refused the same way; there is no fallback to another algorithm.
+ *   - Cost: the array is 256 + 8 * MP_NOALLOC_MAX_M bytes (512.25 KiB).  Every GPU on which the library is loaded keeps
+ *     that much memory until the process exits, used or not.
+ *   - The first call on each device looks the array's device address up (cudaGetSymbolAddress, with that device current,
+ *     under a lock) and remembers it.  Make that first call ahead of time, outside any stream capture.
+ *   - All calls on a device share the one array.  Each call clears the part it needs to start from zero (one memset on
+ *     `stream` ahead of the kernel), so calls issued one after another on one stream, or otherwise ordered on the GPU, are
+ *     independent of each other.  Two calls that can run on the GPU at the same time (different streams without an event
+ *     between them, different host threads) race on the array and return garbage or hang: serialise them. */
+#define MP_NOALLOC_MAX_M 65536
+MP_API mp_status mp_recover_noalloc(const float* psi_t, int N, int M, int64_t ld,
+                             const float* y, float eps, int max_iter,
+                             float* x, float* r, int* n_iter,
+                             int* idx_trace, float* c_trace, void* stream);
+
 /* B signals sharing one dictionary ("all signals are encoded/decoded with the same dictionary").
  * Signal b's result equals mp_recover on (psi_t, Y[b]); signals are independent and a signal that has
  * stopped is frozen (x_b, r_b, n_iter_b no longer change) while the others continue.

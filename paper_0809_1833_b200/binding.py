@@ -50,6 +50,8 @@ lib.mp_normalize_columns.restype = _i
 lib.mp_normalize_columns.argtypes = [_vp, _i, _i, _i64, _vp, _vp]
 lib.mp_recover.restype = _i
 lib.mp_recover.argtypes = [_vp, _i, _i, _i64, _vp, _f, _i, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]
+lib.mp_recover_noalloc.restype = _i
+lib.mp_recover_noalloc.argtypes = [_vp, _i, _i, _i64, _vp, _f, _i, _vp, _vp, _vp, _vp, _vp, _vp]
 lib.mp_recover_batched.restype = _i
 lib.mp_recover_batched.argtypes = [_vp, _i, _i, _i64, _vp, _i64, _i, _f, _i, _vp, _vp, _vp, _vp, _sz, _vp]
 lib.mp_recover_batched_traced.restype = _i
@@ -223,6 +225,35 @@ def mp_recover(psi_t: torch.Tensor, y: torch.Tensor, eps: float, max_iter: int, 
                               _dev(c_trace, torch.float32, "c_trace") if c_trace is not None else None,
                               wp, wb, _stream_ptr(stream)))
     return Recovered(x, r, n_iter, idx_trace, c_trace, workspace)
+
+
+MP_NOALLOC_MAX_M = 65536
+
+
+def mp_recover_noalloc(psi_t: torch.Tensor, y: torch.Tensor, eps: float, max_iter: int, *, x=None, r=None, n_iter=None,
+                       idx_trace=None, c_trace=None, trace: bool = False, stream=None) -> Recovered:
+    """mp_recover without a workspace, for callers that cannot allocate device memory (a plug-in inside a process whose own
+    pool owns the GPU, a loop that must not stall on an allocation): the C call uses a fixed scratch array inside the library
+    and allocates nothing.  M <= MP_NOALLOC_MAX_M; calls that overlap on the GPU race on that array (include/mp_b200.h).
+    Pass x, r, n_iter (and the traces) to keep this wrapper from allocating too: any output left None is a fresh torch tensor."""
+    p, N, M, ld = _dict_args(psi_t)
+    dev = psi_t.device
+    if y.numel() != N:
+        raise ValueError("y must have N elements")
+    x = torch.empty(M, dtype=torch.float32, device=dev) if x is None else x
+    r = torch.empty(N, dtype=torch.float32, device=dev) if r is None else r
+    n_iter = torch.empty(1, dtype=torch.int32, device=dev) if n_iter is None else n_iter
+    if trace and idx_trace is None:
+        idx_trace = torch.empty(max(max_iter, 1), dtype=torch.int32, device=dev)
+    if trace and c_trace is None:
+        c_trace = torch.empty(max(max_iter, 1), dtype=torch.float32, device=dev)
+    with torch.cuda.device(dev):
+        _check(lib.mp_recover_noalloc(p, N, M, ld, _dev(y, torch.float32, "y"), float(eps), int(max_iter),
+                                      _dev(x, torch.float32, "x"), _dev(r, torch.float32, "r"), _dev(n_iter, torch.int32, "n_iter"),
+                                      _dev(idx_trace, torch.int32, "idx_trace") if idx_trace is not None else None,
+                                      _dev(c_trace, torch.float32, "c_trace") if c_trace is not None else None,
+                                      _stream_ptr(stream)))
+    return Recovered(x, r, n_iter, idx_trace, c_trace, None)
 
 
 def mp_recover_batched(psi_t: torch.Tensor, Y: torch.Tensor, eps: float, max_iter: int, *, X=None, R=None, n_iter=None,
