@@ -279,8 +279,13 @@ MP_API const char* mp_last_error(void);
  *                   dictionary is larger than 1.5 MB, else one thread-block cluster per signal (N <= 2048), else sequential;
  *                   1 = tensor-core kernel or MP_ERR_UNSUPPORTED, 2 = one single-signal solve after another,
  *                   3 = one cluster per signal (the mp_recover_many kernel on the shared dictionary) or MP_ERR_UNSUPPORTED
+ *   "info_batched_algo"  (read with mp_get_int) which of 1, 2, 3 the last successful mp_recover_batched call ran.  Auto dispatch falls
+ *                   back from the tensor-core kernel when its cooperative launch is refused; the call still returns MP_OK (the
+ *                   results are the same) but is many times slower, mp_last_error() keeps the refusal and this reads 2 or 3
  *   "batched_coop"  1 (default) = launch the batched kernel with the cooperative attribute (co-residency checked by
- *                   the driver), 0 = plain cluster launch of a grid sized from cudaOccupancyMaxActiveClusters */
+ *                   the driver), 0 = plain cluster launch of a grid sized from cudaOccupancyMaxActiveClusters: only on a device
+ *                   where nothing else runs (profilers that cannot launch cooperative cluster kernels); the library never drops
+ *                   the attribute on its own */
 MP_API mp_status mp_set_int(const char* name, int64_t value);
 MP_API mp_status mp_get_int(const char* name, int64_t* value);
 

@@ -122,7 +122,9 @@ struct DevBuf {
 };
 struct Stream {
     cudaStream_t s = nullptr;
-    ~Stream() { if (s) cudaStreamDestroy(s); }
+    // Synchronise first: an error return must not leave a copy from or to the caller's host buffers in flight (the caller may
+    // free them as soon as the call is back); after a successful call the stream is idle and this costs nothing.
+    ~Stream() { if (s) { (void)cudaStreamSynchronize(s); cudaStreamDestroy(s); } }
 };
 }  // namespace
 
@@ -153,6 +155,7 @@ static int64_t* option_slot(const char* name)
     if (!strcmp(name, "batched_algo")) return &o.batched_algo;
     if (!strcmp(name, "batched_coop")) return &o.batched_coop;
     if (!strcmp(name, "info_algo")) return &o.info_algo;
+    if (!strcmp(name, "info_batched_algo")) return &o.info_batched_algo;
     if (!strcmp(name, "info_l2_pingpong")) return &o.info_l2_pingpong;
     if (!strcmp(name, "info_l2_resident_mb")) return &o.info_l2_resident_mb;
     if (!strcmp(name, "info_l2_dynamic")) return &o.info_l2_dynamic;

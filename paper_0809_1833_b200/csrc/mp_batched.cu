@@ -38,16 +38,19 @@ static mp_status launch_batched_clusters(const BatchedArgs& a, const Workspace& 
 mp_status launch_recover_batched(const BatchedArgs& a, const Workspace& ws, cudaStream_t stream)
 {
     const int64_t algo = options().batched_algo;
-    if (algo == 2) return launch_batched_sequential(a, ws, stream);
-    if (algo == 3) return launch_batched_clusters(a, ws, stream);
+    // "info_batched_algo": which of the three ran (1 tensor-core lock-step, 2 sequential, 3 clusters) -- the only way to see that
+    // auto dispatch left the tensor-core kernel, e.g. after a refused cooperative launch (a 20x slower solve that still succeeds)
+    auto ran = [](int64_t which, mp_status st) { if (st == MP_OK) options().info_batched_algo = which; return st; };
+    if (algo == 2) return ran(2, launch_batched_sequential(a, ws, stream));
+    if (algo == 3) return ran(3, launch_batched_clusters(a, ws, stream));
     const int group = a.B < 64 ? a.B : 64;
     // one signal is not a batch: the single-signal kernels stream the dictionary at the HBM / L2 rate, the lock-step kernel would
     // run a 128-row contraction for one useful row
-    if (algo == 0 && a.B == 1) return launch_batched_sequential(a, ws, stream);
+    if (algo == 0 && a.B == 1) return ran(2, launch_batched_sequential(a, ws, stream));
     // measured (B = 64): 1 MiB dictionary 0.50 ms with clusters against 0.75 ms lock-step; 4 MiB 2.7 against 1.8 ms; 16 MiB 18 against 4.7
-    if (algo == 0 && many_supported(a.N, a.M) && 4.0 * a.N * a.M <= 1.5e6) return launch_batched_clusters(a, ws, stream);
+    if (algo == 0 && many_supported(a.N, a.M) && 4.0 * a.N * a.M <= 1.5e6) return ran(3, launch_batched_clusters(a, ws, stream));
     if (algo == 0 && !batched_tc_supported(a.N, a.M, group))
-        return many_supported(a.N, a.M) ? launch_batched_clusters(a, ws, stream) : launch_batched_sequential(a, ws, stream);
+        return many_supported(a.N, a.M) ? ran(3, launch_batched_clusters(a, ws, stream)) : ran(2, launch_batched_sequential(a, ws, stream));
     for (int b0 = 0; b0 < a.B; b0 += 64) {
         BatchedArgs g = a;
         g.B = a.B - b0 < 64 ? a.B - b0 : 64;
@@ -58,11 +61,12 @@ mp_status launch_recover_batched(const BatchedArgs& a, const Workspace& ws, cuda
         g.idx_trace = a.idx_trace ? a.idx_trace + (int64_t)b0 * a.ldt : nullptr;
         g.c_trace = a.c_trace ? a.c_trace + (int64_t)b0 * a.ldt : nullptr;
         mp_status st = launch_recover_batched_tc(g, ws, nullptr, stream);   // groups reuse the workspace in stream order
-        if (st == MP_ERR_UNSUPPORTED && algo == 0 && b0 == 0)              // e.g. the cooperative cluster launch was refused: nothing ran yet
-            return many_supported(a.N, a.M) ? launch_batched_clusters(a, ws, stream) : launch_batched_sequential(a, ws, stream);
+        if (st == MP_ERR_UNSUPPORTED && algo == 0 && b0 == 0)              // e.g. the cooperative cluster launch was refused: nothing ran yet.
+            // The solve still succeeds on a much slower kernel; mp_last_error() keeps the refusal's text and info_batched_algo says 2 or 3.
+            return many_supported(a.N, a.M) ? ran(3, launch_batched_clusters(a, ws, stream)) : ran(2, launch_batched_sequential(a, ws, stream));
         if (st != MP_OK) return st;
     }
-    return MP_OK;
+    return ran(1, MP_OK);
 }
 
 }  // namespace mp

@@ -660,12 +660,10 @@ mp_status launch_recover_batched_tc(const BatchedArgs& a, const Workspace& ws, f
     at[0].val.clusterDim.x = kTcCluster; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
     at[1].id = cudaLaunchAttributeCooperative;
     at[1].val.cooperative = 1;
-    // Nsight Compute cannot launch a cooperative CLUSTER kernel (it aborts the target with "LaunchFailed") and it serialises
-    // kernels anyway, so under a CUDA injection profiler the same grid goes out as a plain cluster launch: it is sized from
-    // cudaOccupancyMaxActiveClusters and nothing else runs beside it, so all clusters are co-resident as the barriers need.
-    static const bool profiler_injected = getenv("CUDA_INJECTION64_PATH") || getenv("NV_COMPUTE_PROFILER_PERFWORKS_DIR") ||
-                                          getenv("NV_NSIGHT_INJECTION_TRANSPORT_TYPE") || getenv("NVTX_INJECTION64_PATH");
-    cfg.attrs = at; cfg.numAttrs = (options().batched_coop && !profiler_injected) ? 2 : 1;
+    // The cooperative attribute is dropped by the explicit knob "batched_coop" = 0 and by nothing else: the library does not look
+    // at the environment.  (Nsight Compute cannot launch a cooperative CLUSTER kernel; profiling runs and smoke() set the knob,
+    // on a device where nothing else runs, so that the grid sized from cudaOccupancyMaxActiveClusters is co-resident anyway.)
+    cfg.attrs = at; cfg.numAttrs = options().batched_coop ? 2 : 1;
     cudaError_t e = cudaLaunchKernelEx(&cfg, mp_batched_tc_kernel, tm_psi, tm_rs, p);
     if (options().batched_coop && (e == cudaErrorNotSupported || e == cudaErrorCooperativeLaunchTooLarge)) {
         // The kernel spins on hand-rolled grid barriers, so it is only ever launched with the co-residency guarantee of the

@@ -37,8 +37,19 @@ static size_t up256(size_t v) { return (v + 255) / 256 * 256; }
 
 struct DeviceGuard {
     int prev = -1;
-    explicit DeviceGuard(int dev) { cudaGetDevice(&prev); if (prev != dev) cudaSetDevice(dev); else prev = -1; }
+    // dev < 0: a handle whose set-up failed before it learnt its device -- nothing to switch to
+    explicit DeviceGuard(int dev) { if (dev < 0 || cudaGetDevice(&prev) != cudaSuccess || prev == dev) prev = -1; else cudaSetDevice(dev); }
     ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+// Once a copy from or to the caller's HOST buffers has been enqueued, no return path may leave it in flight: the caller is
+// entitled to free or reuse those buffers as soon as the call is back, error or not.  Armed until the call's own final
+// synchronise has succeeded.
+struct SyncOnExit {
+    cudaStream_t s;
+    bool armed = true;
+    explicit SyncOnExit(cudaStream_t stream) : s(stream) {}
+    ~SyncOnExit() { if (armed) (void)cudaStreamSynchronize(s); }
 };
 
 }  // namespace mp
@@ -166,6 +177,7 @@ mp_status mp_recover_batched_host_h(mp_dictionary* h, const float* Y, int64_t ld
     int* dit = traced ? reinterpret_cast<int*>(io + o_it) : nullptr;
     float* dct = traced ? reinterpret_cast<float*>(io + o_ct) : nullptr;
     cudaStream_t s = h->stream;
+    SyncOnExit drain(s);
     MP_CUDA(cudaMemcpy2DAsync(dY, sizeof(float) * (size_t)ldy_d, Y, sizeof(float) * (size_t)ldy, sizeof(float) * (size_t)N, (size_t)B,
                               cudaMemcpyHostToDevice, s));
     if (B == 1)
@@ -183,6 +195,7 @@ mp_status mp_recover_batched_host_h(mp_dictionary* h, const float* Y, int64_t ld
                                                sizeof(float) * (size_t)max_iter, (size_t)B, cudaMemcpyDeviceToHost, s));
     }
     MP_CUDA(cudaStreamSynchronize(s));
+    drain.armed = false;
     return MP_OK;
 }
 

@@ -21,6 +21,7 @@ mp_status cuda_fail(cudaError_t e, const char* what);
 struct Options {
     int64_t algo = 0, warps = 0, slot_bytes = 0, depth = 0, grid = 0, chunk = 64;
     int64_t batched_algo = 0, batched_coop = 1;
+    int64_t info_batched_algo = 0;     // batched path the last mp_recover_batched call took: 1 tensor-core lock-step, 2 sequential, 3 clusters
     int64_t omp_algo = 0, info_omp_algo = 0;   // Orthogonal MP: 0 auto, 1 persistent kernel, 2 stream loop; and the one last used
     int64_t pin_margin_pct = 0;        // with pingpong: percent of a CTA's groups at either end that are never pinned (0 = auto = 10, 100 = none)
     int64_t pingpong = 0;              // register-streaming kernel: reversed item order on odd iterations; 0 = auto (with the residency hints), 1 = off, 2 = on

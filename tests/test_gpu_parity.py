@@ -511,3 +511,19 @@ def test_l2_residency_hints_do_not_change_results(mp, N, M, K):
         mp.mp_set_int("l2_resident_mb", 0)
     for a, b in zip(out, off):
         assert np.array_equal(a, b)
+
+
+def test_info_batched_algo_reports_the_path_taken(mp):
+    """Auto dispatch may leave the tensor-core kernel (tiny dictionary, refused cooperative launch) and still return MP_OK:
+    "info_batched_algo" is how a caller sees which kernel served the last batched call (1 lock-step, 2 sequential, 3 clusters)."""
+    pb = problems.make_problem(problems.custom_config(128, 512, 6, max_iter=40, B=4), seed=9)
+    psi_d, Y_d = dev(pb.psi32), dev(pb.Y)
+    try:
+        for knob, want in ((0, 3), (1, 1), (2, 2), (3, 3)):               # auto: 256 KiB dictionary -> one cluster per signal
+            mp.mp_set_int("batched_algo", knob)
+            res = mp.mp_recover_batched(psi_d, Y_d, pb.cfg.eps, pb.cfg.max_iter)
+            torch.cuda.synchronize()
+            assert mp.mp_get_int("info_batched_algo") == want, (knob, want)
+            assert int(res.n_iter.min().item()) > 0
+    finally:
+        mp.mp_set_int("batched_algo", 0)
