@@ -27,9 +27,29 @@ def deps():
         glob.glob(os.path.join(root, "include", "*.h")) + [os.path.abspath(__file__)]
 
 
+def _up_to_date() -> bool:
+    return os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in deps())
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in deps()):
+    """Processes that import the package together (torchrun ranks, pytest-xdist workers) all come through here.  One of them
+    compiles, under an exclusive lock on build/.lock; the others wait for it and then find the library up to date, so nobody links
+    half-written objects and the library is only ever replaced atomically by the one process that built it."""
+    if not force and _up_to_date():
         return LIB
+    import fcntl
+    os.makedirs(os.path.join(HERE, "build"), exist_ok=True)
+    with open(os.path.join(HERE, "build", ".lock"), "w") as lock:
+        fcntl.flock(lock, fcntl.LOCK_EX)
+        try:
+            if not force and _up_to_date():          # somebody else built it while this process waited
+                return LIB
+            return _build_locked(verbose)
+        finally:
+            fcntl.flock(lock, fcntl.LOCK_UN)
+
+
+def _build_locked(verbose: bool) -> str:
     flags = FLAGS + os.environ.get("MP_B200_EXTRA_NVCC_FLAGS", "").split()
     if verbose:
         flags += ["-Xptxas", "-v"]
@@ -50,8 +70,9 @@ def build(force: bool = False, verbose: bool = False) -> str:
             failed = True
     if failed:
         raise RuntimeError("nvcc failed")
-    subprocess.run([NVCC, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB + ".tmp", *objs, "-cudart", "static"], check=True)
-    os.replace(LIB + ".tmp", LIB)
+    tmp = "%s.%d.tmp" % (LIB, os.getpid())
+    subprocess.run([NVCC, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", tmp, *objs, "-cudart", "static"], check=True)
+    os.replace(tmp, LIB)
     return LIB
 
 

@@ -146,3 +146,36 @@ def test_argument_errors_of_the_dictionary_handle():
     assert lib.mp_recover_host_h(None, ok, 0.1, 1, ok, ok, ok, None, None) == 1
     assert lib.mp_recover_batched_host_h(None, ok, 8, 1, 0.1, 1, ok, ok, ok, None, None, 1) == 1
     assert b"handle" in lib.mp_last_error()
+
+
+def test_concurrent_builds_are_serialised_and_the_waiter_does_not_rebuild(monkeypatch):
+    """Ranks / xdist workers that import the package at the same moment: one compiles under the lock on build/.lock, the others
+    wait and then find the library up to date (paper_0809_1833_b200/build.py).  The compile is replaced by a stub here."""
+    import threading
+    import time
+    from paper_0809_1833_b200 import build as B
+    state = {"built": 0, "inside": 0, "overlap": False}
+
+    def fake_build(verbose):
+        state["inside"] += 1
+        state["overlap"] |= state["inside"] > 1
+        time.sleep(0.3)
+        state["built"] += 1
+        state["inside"] -= 1
+        return B.LIB
+
+    monkeypatch.setattr(B, "_build_locked", fake_build)
+    monkeypatch.setattr(B, "_up_to_date", lambda: state["built"] > 0)
+    threads = [threading.Thread(target=B.build) for _ in range(3)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    assert state["built"] == 1 and not state["overlap"]
+    state["built"] = 0
+    threads = [threading.Thread(target=B.build, kwargs={"force": True}) for _ in range(2)]     # forced: both build, one after the other
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    assert state["built"] == 2 and not state["overlap"]

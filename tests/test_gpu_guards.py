@@ -62,7 +62,7 @@ def test_single_signal_solvers_write_only_what_they_own(mp, N, M, K, algo):
     psi_before = psi.clone()
     y = torch.from_numpy(pb.Y[0]).cuda(); y_before = y.clone()
     fx, fr, fn, fi, fc = Fenced(4 * M), Fenced(4 * N), Fenced(4), Fenced(4 * T), Fenced(4 * T)
-    fw = Fenced(mp.mp_workspace_bytes(N, M, 1) + 256)
+    fw = Fenced(mp.mp_workspace_bytes(N, M, 1))   # exactly the declared size: the fence starts where the workspace ends
     mp.mp_set_int("algo", algo)
     try:
         res = mp.mp_recover(psi, y, pb.cfg.eps, T, x=fx.view(torch.float32, M), r=fr.view(torch.float32, N),
@@ -88,7 +88,7 @@ def test_batched_solvers_write_only_what_they_own(mp, N, M, K, B, algo):
     psi = padded(pb.psi32, (N + 3) // 4 * 4 + 4); psi_before = psi.clone()
     Y = padded(pb.Y, (N + 3) // 4 * 4); Y_before = Y.clone()
     fX, fR, fn, fi, fc = Fenced(4 * B * M), Fenced(4 * B * N), Fenced(4 * B), Fenced(4 * B * T), Fenced(4 * B * T)
-    fw = Fenced(mp.mp_workspace_bytes(N, M, B) + 256)
+    fw = Fenced(mp.mp_workspace_bytes(N, M, B))
     mp.mp_set_int("batched_algo", algo)
     try:
         res = mp.mp_recover_batched(psi, Y, pb.cfg.eps, T, X=fX.view(torch.float32, B * M).view(B, M),
@@ -115,7 +115,7 @@ def test_workspaces_of_the_widened_entry_points_are_respected(mp, N, M, K):
     lib = mp.binding.lib
     psi = padded(pb.psi32, (N + 3) // 4 * 4 + 4); psi_before = psi.clone()
     y = torch.from_numpy(pb.Y[0]).cuda()
-    fw = Fenced(lib.mp_workspace_bytes_omp(N, M, T) + 256)
+    fw = Fenced(lib.mp_workspace_bytes_omp(N, M, T))
     for omp_algo in (1, 2):
         mp.mp_set_int("omp_algo", omp_algo)
         try:
@@ -126,13 +126,13 @@ def test_workspaces_of_the_widened_entry_points_are_respected(mp, N, M, K):
         assert fw.intact(), f"mp_recover_omp (omp_algo {omp_algo}) wrote outside its workspace"
     mp.mp_set_int("omp_algo", 0)
     psi64 = padded(pb.psi32.astype(np.float64), (N + 1) // 2 * 2 + 2); psi64_before = psi64.clone()
-    fw = Fenced(lib.mp_workspace_bytes_f64(N, M) + 256)
+    fw = Fenced(lib.mp_workspace_bytes_f64(N, M))
     mp.mp_recover_f64(psi64, y.double(), pb.cfg.eps, T, trace=True, workspace=fw.inner)
     torch.cuda.synchronize()
     assert fw.intact(), "mp_recover_f64 wrote outside its workspace"
     assert torch.equal(psi64.nan_to_num(), psi64_before.nan_to_num())
     Y = padded(pb.Y, (N + 3) // 4 * 4)
-    fw = Fenced(lib.mp_workspace_bytes_many(N, M, 3) + 256)
+    fw = Fenced(lib.mp_workspace_bytes_many(N, M, 3))
     try:
         mp.mp_recover_many(psi, Y, pb.cfg.eps, T, trace=True, workspace=fw.inner)
         torch.cuda.synchronize()
