@@ -32,6 +32,22 @@ def pytest_collection_modifyitems(config, items):
             it.add_marker(skip)
 
 
+def pytest_sessionfinish(session, exitstatus):
+    """The two state-drift allowances of the grading (R14b, R16b) are for rare cases: a session that needs them more often than
+    tests/grading.py expects fails as a whole, even if every single grade passed."""
+    try:
+        import grading
+    except Exception:
+        return
+    g1 = sum(1 for g in grading.LOG if g["g1_allowance_used"])
+    nd = sum(1 for g in grading.LOG if g["n_iter_drift_used"])
+    if g1 > grading.G1_ALLOWANCE_MAX_USES or nd > grading.N_ITER_DRIFT_MAX_USES:
+        print(f"\ngrading: state-drift allowances used too often (G1 {g1} > {grading.G1_ALLOWANCE_MAX_USES} or "
+              f"n_iter {nd} > {grading.N_ITER_DRIFT_MAX_USES}): failing the session")
+        if exitstatus == 0:
+            session.exitstatus = 1
+
+
 def pytest_terminal_summary(terminalreporter, exitstatus, config):
     """How often the G1 state-drift allowance (reading R14b) was needed, and the worst observed errors of the session."""
     try:

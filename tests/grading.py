@@ -38,6 +38,18 @@ def c_tol_tensor_core(N: int) -> float:
 NORM_TOL = 1e-4     # north_star: final ||r|| within 1e-4 relative
 X_TOL = 1e-4        # north_star: ||x_gpu - x_ref|| / ||x_ref||
 
+# Caps on the two state-drift allowances (readings R14b, R16b), so that neither can grow without anybody noticing:
+#   * the drift itself is bounded by what G3 tolerates: d_{s+1} = (I - psi_s psi_s^T) d_s + e_s psi_s with e_s = c_gpu,s - <r_image,s, psi_s>
+#     (the oracle's free-running step is its own correlation, which already contains <d_s, psi_s>), a projection is non-expansive,
+#     hence ||d|| <= sum_s |e_s| <= sum_s c_tol ||r_s||.  Asserted below on the replay's norms, after G3.
+#   * ceilings with about 2x headroom over the worst case of the full GPU session (1425 grades: G1 allowance used 33 times, largest
+#     8.3e-3 at an oracle gap of 7.1e-3; n_iter drift used once, 1.2e-3 of the threshold).  Beyond them a run is looked at by hand.
+#   * the session as a whole may use them at most G1_ALLOWANCE_MAX_USES / N_ITER_DRIFT_MAX_USES times (tests/conftest.py).
+G1_ALLOWANCE_CEILING = 2e-2
+N_ITER_DRIFT_CEILING = 5e-3        # ||d|| / (eps ||y||)
+G1_ALLOWANCE_MAX_USES = 50
+N_ITER_DRIFT_MAX_USES = 3
+
 # Every grade of the session, so that the use of the G1 allowance and the worst observed errors are visible
 # (tests/conftest.py prints the summary and writes it to gpurun_out/grading_summary.json when that folder exists).
 LOG: list[dict] = []
@@ -106,6 +118,10 @@ def grade_single(psi32: np.ndarray, y32: np.ndarray, eps: float, max_iter: int,
         g1_gap = float(ref.gap[first_div])
         g1_used = bool(g1_gap > GAP_TOL)
         allowance = GAP_TOL + g1_allow
+        g1_drift = float(np.linalg.norm(d))
+        assert not g1_used or g1_allow <= G1_ALLOWANCE_CEILING, (
+            f"free-running divergence at t={first_div} needs a state-drift allowance of {g1_allow:.3e} > ceiling {G1_ALLOWANCE_CEILING} "
+            f"(oracle gap {g1_gap:.3e}): the step errors have grown, look at G3's margins")
         assert ref.gap[first_div] <= allowance, (
             f"free-running sequences diverge at t={first_div} where the oracle's top-two gap is {ref.gap[first_div]:.3e} "
             f"> {GAP_TOL} + state-drift allowance {allowance - GAP_TOL:.3e}")
@@ -121,6 +137,9 @@ def grade_single(psi32: np.ndarray, y32: np.ndarray, eps: float, max_iter: int,
     c_err = np.abs(c_gpu - rp.c_at_idx) / np.maximum(rp.rnorm[:t_gpu], np.finfo(np.float64).tiny) if t_gpu else np.zeros(0)
     max_c_err = float(c_err.max()) if t_gpu else 0.0
     assert max_c_err <= c_tol, f"step value error {max_c_err:.3e} ||r|| at t={int(c_err.argmax())} exceeds {c_tol}"
+    if first_div >= 0:                                     # the drift G1 allowed for is within what G3 tolerates (see the caps above)
+        bound = c_tol * float(np.sum(rp.rnorm[:first_div]))
+        assert g1_drift <= bound * (1.0 + 1e-6) + 1e-300, f"state drift ||d|| = {g1_drift:.3e} exceeds the G3-derived bound {bound:.3e}"
 
     # ---- G4 final residual and coefficients ---------------------------------------------------------------------
     nr_gpu = float(np.linalg.norm(r_gpu))
@@ -156,6 +175,10 @@ def grade_single(psi32: np.ndarray, y32: np.ndarray, eps: float, max_iter: int,
             nd = float(np.linalg.norm(d))
             nd_rel = nd / thr if thr > 0 else 0.0
             nd_used = bool(abs(edge - thr) > NORM_TOL * thr)
+            bound = c_tol * float(np.sum(rp.rnorm[:e]))
+            assert nd <= bound * (1.0 + 1e-6) + 1e-300, f"state drift ||d|| = {nd:.3e} exceeds the G3-derived bound {bound:.3e}"
+            assert not nd_used or nd_rel <= N_ITER_DRIFT_CEILING, (
+                f"n_iter differs by one with a state drift of {nd_rel:.3e} of the threshold > ceiling {N_ITER_DRIFT_CEILING}")
             assert abs(edge - thr) <= NORM_TOL * thr + nd, (
                 f"n_iter differs by one away from the stopping threshold: | ||r_ref|| - thr | = {abs(edge - thr):.3e}, "
                 f"NORM_TOL * thr = {NORM_TOL * thr:.3e}, state drift ||d|| = {nd:.3e}")

@@ -72,3 +72,35 @@ def test_reference_arm_rank0_prints_contract_line():
 def test_reference_arm_other_ranks_exit_silently():
     p = _run_reference(1, 2)
     assert p.returncode == 0 and p.stdout.strip() == ""
+
+
+def test_grading_drift_caps_hold_for_a_run_within_g3_and_catch_one_outside():
+    """tests/grading.py caps the state drift behind R14b / R16b by what G3 tolerates (||d|| <= sum_s c_tol ||r_s||) and by fixed
+    ceilings.  A stand-in for a GPU run is made on the host -- the MP trajectory with every step perturbed by up to half the G3
+    tolerance, as fp32 dot products would -- and must be graded clean with the caps in place; the session-level use counts must
+    leave room for what the full GPU session is known to need."""
+    import numpy as np
+    import grading
+    import oracle
+    import problems
+    pb = problems.make_problem(problems.custom_config(96, 300, 8, eps=1e-5, max_iter=40), seed=5)
+    y = pb.Y[0]
+    ref = oracle.mp(pb.psi32, y.astype(np.float64), float(np.float32(pb.cfg.eps)), pb.cfg.max_iter, 1)
+    rng = np.random.default_rng(0)
+    # replay the oracle's atoms with perturbed steps: c_s = <r_s, psi> + 0.5 * C_TOL * ||r_s|| * u, u in [-1, 1]
+    r = y.astype(np.float64).copy()
+    idx, c = [], []
+    ny = np.linalg.norm(r)
+    thr = float(np.float32(pb.cfg.eps)) * ny
+    x = np.zeros(pb.cfg.M)
+    while np.linalg.norm(r) > thr and len(idx) < pb.cfg.max_iter:
+        corr = pb.psi32.astype(np.float64) @ r
+        i = int(np.argmax(np.abs(corr)))
+        step = float(np.float32(corr[i] + 0.5 * grading.C_TOL * np.linalg.norm(r) * rng.uniform(-1, 1)))
+        idx.append(i); c.append(step)
+        x[i] += step
+        r -= step * pb.psi32[i].astype(np.float64)
+    g = grading.grade_single(pb.psi32, y, pb.cfg.eps, pb.cfg.max_iter, x.astype(np.float32), r.astype(np.float32), len(idx),
+                             np.array(idx, np.int32), np.array(c, np.float32), ref=ref, nthreads=1)
+    assert g.max_c_err <= grading.C_TOL and g.g1_allowance <= grading.G1_ALLOWANCE_CEILING
+    assert grading.G1_ALLOWANCE_MAX_USES >= 33 and grading.N_ITER_DRIFT_MAX_USES >= 1      # the full GPU session's counts fit
