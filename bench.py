@@ -270,7 +270,35 @@ class Workload:
                 "its_per_step": int(self.n_d.sum().item()), "its_max": int(self.n_d.max().item())}
 
 
-def roofline_of(mp, cfg, m, traffic_per_it=None, traffic_src=None):
+def probe_read_gbs(torch, mp, dev, nbytes, passes, reps=3):
+    """GB/s of the library's read-only streaming diagnostic (mp_probe_read: the item loop of the single-signal kernel, no barrier,
+    no argmax) over a buffer of `nbytes`: the L2 read rate when the buffer fits in L2, the HBM read rate when it is much larger.
+    Outside every timed region of the metric; best of `reps` after one warm-up launch."""
+    unit = 148 * 8192
+    nbytes = max(unit, (int(nbytes) + unit - 1) // unit * unit)
+    buf = torch.ones(nbytes // 4, dtype=torch.float32, device=dev)
+    sink = torch.zeros(1, dtype=torch.float32, device=dev)
+    stream = torch.cuda.current_stream()
+    mp.mp_probe_read(buf, max(1, passes // 4), sink=sink)
+    torch.cuda.synchronize()
+    best, read = 0.0, 0
+    for _ in range(reps):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        read = mp.mp_probe_read(buf, passes, sink=sink)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        best = max(best, read / (e0.elapsed_time(e1) * 1e-3) / 1e9)
+    del buf
+    torch.cuda.empty_cache()
+    return {"gbs": best, "buffer_bytes": nbytes, "passes": passes, "bytes_read_per_launch": read,
+            "source": "mp_probe_read (read-only 128-bit streaming loop of the single-signal kernel, one CTA per SM), CUDA events, best of %d, this run" % reps}
+
+
+L2_RESIDENT_MAX_BYTES = 100e6      # dictionaries up to here are served by the 126 MB L2 after the first iteration (DESIGN.md section 5)
+
+
+def roofline_of(mp, cfg, m, traffic_per_it=None, traffic_src=None, l2_probe=None):
     """The roofline object of the dominant kernel for one measured workload."""
     N, M, B = cfg.N, cfg.M, cfg.B
     its_max, solve_ms = m["its_max"], m["solve_ms"]
@@ -289,12 +317,17 @@ def roofline_of(mp, cfg, m, traffic_per_it=None, traffic_src=None):
     # (SURVEY.md 8(d)); the batched loop runs until its slowest signal stops.
     alg_bytes = its_max * (4.0 * N * M + 4.0 * N * B)
     achieved = alg_bytes / (solve_ms * 1e-3) / 1e9
-    streaming = 4.0 * N * M > 126e6
-    rl = {"bound": "hbm", "regime": "hbm-streaming" if streaming else "l2-resident (frac is against the HBM peak: > 1 means served from L2)",
+    streaming = 4.0 * N * M > L2_RESIDENT_MAX_BYTES
+    rl = {"bound": "hbm", "regime": "hbm-streaming" if streaming else "l2-resident",
           "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
           "traffic": traffic_per_it * its_max if traffic_per_it else None, "traffic_source": traffic_src, "peak_source": peak_src,
           "kernel": mp_kernel_name(mp, B > 1), "algorithmic_bytes_per_launch": alg_bytes, "kernel_ms": solve_ms,
           "us_per_iteration": 1e3 * solve_ms / max(its_max, 1)}
+    if not streaming and l2_probe:
+        # cache-resident regime (north_star: "or L2 bandwidth when Psi fits in L2"): the roofline is the L2 read rate, measured in
+        # this run by the library's read-only probe over a buffer of the dictionary's own size
+        rl.update({"bound": "l2", "peak": l2_probe["gbs"], "frac": achieved / l2_probe["gbs"], "peak_source": l2_probe["source"],
+                   "l2_probe": l2_probe, "frac_vs_hbm_peak": achieved / peak, "hbm_peak": peak})
     if traffic_per_it and streaming:
         rl["dram_achieved"] = traffic_per_it * its_max / (solve_ms * 1e-3) / 1e9
         rl["dram_frac"] = rl["dram_achieved"] / peak
@@ -310,7 +343,7 @@ def main():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--no-extra", action="store_true", help="skip the no-hint leg and the cfg2 / cfg5 / cfg4_32768 figures of the default run")
+    ap.add_argument("--no-extra", action="store_true", help="skip the no-hint leg, the read probe and the cfg1 / cfg2 / cfg4 sweep / cfg5 figures of the default run")
     ap.add_argument("--max-iter", type=int, default=None, help="override the config's iteration cap (profiling runs)")
     ap.add_argument("--f64", action="store_true", help="double-precision path (mp_recover_f64) on the same workload shape")
     ap.add_argument("--omp", action="store_true", help="Orthogonal MP (mp_recover_omp) on the same workload")
@@ -372,11 +405,15 @@ def main():
     per_it = per_it_off = tsrc = None
     if args.config == "cfg3" and not args.knob and args.max_iter is None and mp.mp_get_int("info_algo") == 3:
         per_it, per_it_off, tsrc = ncu_traffic(mp_kernel_name(mp, False))
-    roofline = roofline_of(mp, cfg, m, per_it, tsrc)
+    l2p = None
+    if B == 1 and world == 1 and 4.0 * N * M <= L2_RESIDENT_MAX_BYTES:          # cache-resident config: roofline = the L2 read rate at this size
+        l2p = probe_read_gbs(torch, mp, dev, 4.0 * N * M, passes=int(max(50, min(4000, 2.5e10 / (4.0 * N * M)))))
+    roofline = roofline_of(mp, cfg, m, per_it, tsrc, l2_probe=l2p)
     if mp.mp_get_int("info_algo") == 3:
         roofline["l2_plan"] = {"reversed_order_on_odd_iterations": bool(mp.mp_get_int("info_l2_pingpong")),
                                "pinned_mb": int(mp.mp_get_int("info_l2_resident_mb")),
-                               "items_drawn_from_counter": bool(mp.mp_get_int("info_l2_dynamic"))}
+                               "items_drawn_from_counter": bool(mp.mp_get_int("info_l2_dynamic")),
+                               "l2_bytes": int(mp.mp_get_int("info_l2_bytes"))}   # cudaDevAttrL2CacheSize: the plan's thresholds are fractions of it
     if per_it and "dram_frac" in roofline:
         # frac can exceed 1: ~88 MB of the dictionary are pinned in L2 (L2::evict_last loads) and odd iterations visit the rows in
         # reverse order, so that the rows read last are read first again: the kernel moves fewer HBM bytes per iteration than 4NM.
@@ -403,6 +440,11 @@ def main():
                                "dram_frac": ro.get("dram_frac"), "steps": 3, "warmup": 3, "clocks": mo["clocks"],
                                "knob": "l2_resident_mb=1 pingpong=1 (no pinned rows, same visiting order every iteration): all 4NM bytes per iteration come from HBM"}
 
+    if default_run:
+        # the same-run anchor of the 1.02 / 1.47: what a read-only stream of the kernel's own access pattern gets from HBM (1 GiB buffer)
+        hb = probe_read_gbs(torch, mp, dev, 1 << 30, passes=8)
+        roofline["read_ceiling_hbm"] = {**hb, "frac_of_copy_peak": hb["gbs"] / roofline["peak"]}
+
     # ---- e2e: the host-buffer C-ABI call, H2D of the dictionary and y and D2H of x, r, n_iter inside the timed region ----
     e2e = None
     if not args.no_e2e:
@@ -417,8 +459,10 @@ def main():
         del wl
         torch.cuda.empty_cache()
         extra = {}
-        for name in ("cfg2", "cfg4_32768", "cfg5"):
-            extra[name] = extra_leg(torch, mp, synth.config(name), local, dev)
+        # the whole size sweep of BASELINE.json configs[3] (4 MiB ... 1 GiB, across the L2-to-HBM transition), cfg1, cfg2 and cfg5
+        for name in ("cfg1", "cfg2", "cfg4_2048", "cfg4_4096", "cfg4_8192", "cfg4_16384", "cfg4_32768", "cfg5"):
+            small = name in ("cfg1", "cfg4_2048", "cfg4_4096", "cfg4_16384")
+            extra[name] = extra_leg(torch, mp, synth.config(name), local, dev, steps=3 if small else 5)
 
     if rank == 0:
         print(json.dumps({
@@ -433,17 +477,29 @@ def main():
 
 
 def extra_leg(torch, mp, cfg, local, dev, steps=5, warmup=3):
-    """One of the other regimes (cfg2: L2-resident; cfg5: batched tensor-core; cfg4_32768: 1 GiB from HBM), same protocol as
-    the headline: W warm-ups, K timed steps, CUDA events, nvidia-smi clocks during its own timed region."""
+    """One of the other regimes (cfg1, cfg2, the cfg4 sizes: L2-resident up to 64 MiB, 1 GiB from HBM; cfg5: batched tensor-core),
+    same protocol as the headline: W warm-ups, K timed steps, CUDA events, nvidia-smi clocks during its own timed region (one retry
+    if that region saw a slowdown flag).  L2-resident sizes are stated against the L2 read rate the probe gives at their own size."""
     wl = Workload(torch, mp, cfg, 1, dev)
     m = wl.timed(steps, warmup, local)
-    rl = roofline_of(mp, cfg, m)
+    algo = int(mp.mp_get_int("info_algo")) if cfg.B == 1 else None
+    probe = None
+    if cfg.B == 1 and 4.0 * cfg.N * cfg.M <= L2_RESIDENT_MAX_BYTES:
+        nbytes = 4.0 * cfg.N * cfg.M
+        probe = probe_read_gbs(torch, mp, dev, nbytes, passes=int(max(50, min(4000, 2.5e10 / nbytes))))
+    rl = roofline_of(mp, cfg, m, l2_probe=probe)
     out = {"workload": workload_name(cfg), "bound": rl["bound"], "frac": rl["frac"], "achieved": rl["achieved"], "peak": rl["peak"],
-           "unit": rl["unit"], "kernel": rl["kernel"], "iterations_per_step": m["its_per_step"], "steps": steps, "warmup": warmup,
-           "ms_per_solve": m["solve_ms"], "clocks": m["clocks"],
+           "unit": rl["unit"], "peak_source": rl["peak_source"], "kernel": rl["kernel"], "iterations_per_step": m["its_per_step"],
+           "steps": steps, "warmup": warmup, "ms_per_solve": m["solve_ms"], "clocks": m["clocks"],
            "us_per_iteration": rl.get("us_per_iteration", rl.get("us_per_lockstep_iteration"))}
-    if "regime" in rl:
-        out["regime"] = rl["regime"]
+    for k in ("regime", "frac_vs_hbm_peak", "l2_probe"):
+        if k in rl:
+            out[k] = rl[k]
+    if algo is not None:
+        out["algo"] = algo
+        if algo == 4:
+            out["note"] = ("one 16-CTA cluster holds the dictionary in shared memory for the whole solve (no L2 traffic for Psi after "
+                           "the first pass): the iteration is bound by the exchange inside the cluster, frac is bytes/time against the L2 rate for scale")
     if cfg.B > 1:
         out["signal_iterations_per_s"] = m["its_per_step"] / (m["solve_ms"] * 1e-3)
     del wl

@@ -266,6 +266,9 @@ MP_API const char* mp_last_error(void);
  *                   dictionaries above 140 MB (none below), and "pin_margin_pct" (0 = auto = 10, 100 = none) percent of a CTA's
  *                   rows at either end of its share are never pinned: the reversed order re-reads them soonest
  *   "info_l2_pingpong", "info_l2_resident_mb", "info_l2_dynamic"  (read with mp_get_int) the L2 plan the last algo-3 launch used
+ *   "l2_bytes"      the L2 size the automatic plan is made for: 0 (default) = the device's cudaDevAttrL2CacheSize; the megabyte figures
+ *                   above are those of a 126.5 MiB L2 and scale with it (they are fractions of the L2); another value = plan as if the
+ *                   L2 had that many bytes (tests; a co-tenant that owns part of the L2).  "info_l2_bytes": the size the last plan used
  *   "balance"       algo 3, shares of >= 8 work items per warp (dictionaries that stream from HBM): 0 (default) = the warps of a CTA
  *                   draw their work items from a counter, so a CTA finishes when its share is done and not when its slowest warp
  *                   is (results do not depend on it), 1 = plain round-robin
@@ -288,6 +291,17 @@ MP_API const char* mp_last_error(void);
  *                   the attribute on its own */
 MP_API mp_status mp_set_int(const char* name, int64_t value);
 MP_API mp_status mp_get_int(const char* name, int64_t* value);
+
+/* Read-only streaming diagnostic (not part of the method): the ceiling the correlation pass (Eq. 9) is measured against.
+ * Reads the first k * 8 KiB * (number of SMs) bytes of buf (k = the largest integer that fits in `bytes`) `passes` times with the
+ * access pattern of the single-signal kernel -- one CTA per SM on a contiguous share, 16 independent 128-bit loads per lane in flight,
+ * four FMAs per load -- and nothing else (no shared memory, no barrier, no argmax).  A buffer that fits in L2 read for many passes
+ * gives the L2 read rate, the roofline of the cache-resident configurations; a buffer much larger than L2 gives the HBM read rate.
+ *   buf         in   device, 16-byte aligned, `bytes` long (contents irrelevant but finite values keep the FMAs cheap)
+ *   sink        out  device, 1 float: receives a sum that only exists to keep the loads alive (accumulated with atomicAdd)
+ *   bytes_read  out  HOST pointer, nullable: bytes the launch reads in total (all passes), for the caller's GB/s
+ * Asynchronous on `stream`; the caller times it (CUDA events).  MP_ERR_INVALID_ARG if the buffer is smaller than 8 KiB per SM. */
+MP_API mp_status mp_probe_read(const void* buf, size_t bytes, int passes, float* sink, unsigned long long* bytes_read, void* stream);
 
 /* Number of kernels the library has launched on behalf of this process so far (for bench.py's gpu_launches). */
 MP_API int64_t mp_launch_count(void);

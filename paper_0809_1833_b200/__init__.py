@@ -9,7 +9,7 @@ library is missing and cannot be built -- there is no CPU fallback.
 """
 _BINDING_NAMES = {
     "mp_normalize_columns", "mp_recover", "mp_recover_noalloc", "MP_NOALLOC_MAX_M", "mp_recover_batched", "mp_recover_host", "mp_recover_batched_host",
-    "mp_workspace_bytes", "mp_correlate_batched", "mp_encode_sparse", "mp_reconstruction_error", "mp_recover_f64", "mp_normalize_columns_f64", "mp_recover_omp", "mp_pack_signs", "mp_recover_signs", "mp_recover_many", "mp_recover_signs_many", "mp_transpose_rowmajor", "mp_set_int", "mp_get_int", "mp_last_error", "mp_launch_count",
+    "mp_workspace_bytes", "mp_probe_read", "mp_correlate_batched", "mp_encode_sparse", "mp_reconstruction_error", "mp_recover_f64", "mp_normalize_columns_f64", "mp_recover_omp", "mp_pack_signs", "mp_recover_signs", "mp_recover_many", "mp_recover_signs_many", "mp_transpose_rowmajor", "mp_set_int", "mp_get_int", "mp_last_error", "mp_launch_count",
     "mp_dictionary_create", "mp_dictionary_destroy", "mp_recover_host_h", "mp_recover_batched_host_h", "Dictionary",
     "MPError", "Recovered", "MP_OK", "MP_ERR_INVALID_ARG", "MP_ERR_CUDA", "MP_ERR_UNSUPPORTED", "MP_ERR_WORKSPACE",
 }

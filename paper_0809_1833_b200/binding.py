@@ -94,6 +94,8 @@ lib.mp_set_int.restype = _i
 lib.mp_set_int.argtypes = [C.c_char_p, _i64]
 lib.mp_get_int.restype = _i
 lib.mp_get_int.argtypes = [C.c_char_p, C.POINTER(_i64)]
+lib.mp_probe_read.restype = _i
+lib.mp_probe_read.argtypes = [_vp, _sz, _i, _vp, C.POINTER(C.c_ulonglong), _vp]
 lib.mp_launch_count.restype = _i64
 lib.mp_launch_count.argtypes = []
 lib.mp_recover_host.restype = _i
@@ -133,6 +135,20 @@ def mp_get_int(name: str) -> int:
 
 def mp_launch_count() -> int:
     return lib.mp_launch_count()
+
+
+def mp_probe_read(buf: torch.Tensor, passes: int, *, sink: torch.Tensor | None = None, stream=None) -> int:
+    """The read-only streaming diagnostic (include/mp_b200.h): enqueues `passes` reads of the device tensor `buf` and returns the
+    number of bytes the launch reads; the caller times it with CUDA events."""
+    if not (buf.is_cuda and buf.is_contiguous()):
+        raise TypeError("buf must be a contiguous CUDA tensor")
+    sink = torch.zeros(1, dtype=torch.float32, device=buf.device) if sink is None else sink
+    n = C.c_ulonglong(0)
+    with torch.cuda.device(buf.device):
+        _check(lib.mp_probe_read(buf.data_ptr(), buf.numel() * buf.element_size(), int(passes), _dev(sink, torch.float32, "sink"),
+                                 C.byref(n), _stream_ptr(stream)))
+    buf._mp_sink = sink                 # keep the sink alive until the stream has run the kernel
+    return n.value
 
 
 def mp_workspace_bytes(N: int, M: int, B: int = 1) -> int:

@@ -46,10 +46,22 @@ mp_status device_info(DeviceInfo* out)
         MP_CUDA(cudaDeviceGetAttribute(&d.sm_count, cudaDevAttrMultiProcessorCount, dev));
         MP_CUDA(cudaDeviceGetAttribute(&d.smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
         MP_CUDA(cudaDeviceGetAttribute(&d.coop, cudaDevAttrCooperativeLaunch, dev));
+        MP_CUDA(cudaDeviceGetAttribute(&d.l2_bytes, cudaDevAttrL2CacheSize, dev));
         cache = d;
     }
     *out = cache;
     return MP_OK;
+}
+
+double l2_scale()
+{
+    double bytes = (double)options().l2_bytes;
+    if (!(bytes > 0.0)) {
+        DeviceInfo di;
+        bytes = (device_info(&di) == MP_OK && di.l2_bytes > 0) ? (double)di.l2_bytes : kL2TunedBytes;
+    }
+    options().info_l2_bytes = (int64_t)bytes;
+    return bytes / kL2TunedBytes;
 }
 
 static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
@@ -142,7 +154,7 @@ const char* mp_last_error(void) { return g_err; }
 
 int64_t mp_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
 
-static int64_t* option_slot(const char* name)
+static std::atomic<int64_t>* option_slot(const char* name)
 {
     Options& o = options();
     if (!name) return nullptr;
@@ -163,6 +175,8 @@ static int64_t* option_slot(const char* name)
     if (!strcmp(name, "info_omp_algo")) return &o.info_omp_algo;
     if (!strcmp(name, "l2_resident_mb")) return &o.l2_resident_mb;
     if (!strcmp(name, "l2_demote")) return &o.l2_demote;
+    if (!strcmp(name, "l2_bytes")) return &o.l2_bytes;
+    if (!strcmp(name, "info_l2_bytes")) return &o.info_l2_bytes;
     if (!strcmp(name, "balance")) return &o.balance;
     if (!strcmp(name, "pingpong")) return &o.pingpong;
     if (!strcmp(name, "pin_margin_pct")) return &o.pin_margin_pct;
@@ -182,7 +196,7 @@ static int64_t* option_slot(const char* name)
 
 mp_status mp_set_int(const char* name, int64_t value)
 {
-    int64_t* s = option_slot(name);
+    std::atomic<int64_t>* s = option_slot(name);
     if (!s) return fail(MP_ERR_INVALID_ARG, "unknown option '%s'", name ? name : "(null)");
     if (value < 0) return fail(MP_ERR_INVALID_ARG, "option '%s' must be >= 0", name);
     *s = value;
@@ -191,7 +205,7 @@ mp_status mp_set_int(const char* name, int64_t value)
 
 mp_status mp_get_int(const char* name, int64_t* value)
 {
-    int64_t* s = option_slot(name);
+    std::atomic<int64_t>* s = option_slot(name);
     if (!s || !value) return fail(MP_ERR_INVALID_ARG, "unknown option or null output");
     *value = *s;
     return MP_OK;

@@ -1,6 +1,7 @@
 // mp_internal.h -- host-side plumbing shared by the translation units of libmp_b200.so.
 #pragma once
 #include <cuda_runtime.h>
+#include <atomic>
 #include <stddef.h>
 #include <stdint.h>
 
@@ -18,30 +19,41 @@ mp_status cuda_fail(cudaError_t e, const char* what);
     } while (0)
 
 // ---- process-wide knobs (mp_set_int) ---------------------------------------------------------------------
+// Atomics: the header lets several host threads issue solves at once, and every launch records its plan in the info_* fields
+// (and reads the knobs); plain int64_t fields would make that a data race.  The VALUES are still process-wide: with solves
+// running on several threads an info_* read returns the plan of whichever launch wrote last.
 struct Options {
-    int64_t algo = 0, warps = 0, slot_bytes = 0, depth = 0, grid = 0, chunk = 64;
-    int64_t batched_algo = 0, batched_coop = 1;
-    int64_t info_batched_algo = 0;     // batched path the last mp_recover_batched call took: 1 tensor-core lock-step, 2 sequential, 3 clusters
-    int64_t omp_algo = 0, info_omp_algo = 0;   // Orthogonal MP: 0 auto, 1 persistent kernel, 2 stream loop; and the one last used
-    int64_t pin_margin_pct = 0;        // with pingpong: percent of a CTA's groups at either end that are never pinned (0 = auto = 10, 100 = none)
-    int64_t pingpong = 0;              // register-streaming kernel: reversed item order on odd iterations; 0 = auto (with the residency hints), 1 = off, 2 = on
-    int64_t balance = 0;               // register-streaming kernel: 0 = warps draw their items from a counter when the shares are long, 1 = plain round-robin
-    int64_t l2_demote = 0;             // 0 = pinned rows are demoted to evict_normal when a solve ends, 1 = left pinned (measurements)
-    int64_t l2_resident_mb = 0;        // register-streaming kernel: MB of dictionary kept in L2 with evict_last (0 = auto, 1 = off)
-    int64_t many_cluster = 0, many_threads = 0, many_stat = 0, many_l2_mb = 0;   // cluster-per-problem kernel: CTAs per problem (0 auto), threads per CTA (0 auto), 2 = never stationary
-    int64_t info_many_cluster = 0, info_many_stat = 0, info_many_clusters = 0, info_many_threads = 0;   // plan of its last launch
-    int64_t info_l2_pingpong = 0, info_l2_resident_mb = 0, info_l2_dynamic = 0;   // L2 plan of the last register-streaming launch (read-only use)
-    int64_t info_algo = 0;             // kernel the last mp_recover call used (1, 2 or 3)
-    int64_t info_tc_clusters = 0, info_tc_at = 0, info_tc_stages = 0;   // plan of the last batched tensor-core launch (read-only use)
+    std::atomic<int64_t> algo{0}, warps{0}, slot_bytes{0}, depth{0}, grid{0}, chunk{64};
+    std::atomic<int64_t> batched_algo{0}, batched_coop{1};
+    std::atomic<int64_t> info_batched_algo{0};     // batched path the last mp_recover_batched call took: 1 tensor-core lock-step, 2 sequential, 3 clusters
+    std::atomic<int64_t> omp_algo{0}, info_omp_algo{0};   // Orthogonal MP: 0 auto, 1 persistent kernel, 2 stream loop; and the one last used
+    std::atomic<int64_t> pin_margin_pct{0};        // with pingpong: percent of a CTA's groups at either end that are never pinned (0 = auto = 10, 100 = none)
+    std::atomic<int64_t> pingpong{0};              // register-streaming kernel: reversed item order on odd iterations; 0 = auto (with the residency hints), 1 = off, 2 = on
+    std::atomic<int64_t> balance{0};               // register-streaming kernel: 0 = warps draw their items from a counter when the shares are long, 1 = plain round-robin
+    std::atomic<int64_t> l2_demote{0};             // 0 = pinned rows are demoted to evict_normal when a solve ends, 1 = left pinned (measurements)
+    std::atomic<int64_t> l2_resident_mb{0};        // register-streaming kernel: MB of dictionary kept in L2 with evict_last (0 = auto, 1 = off)
+    std::atomic<int64_t> many_cluster{0}, many_threads{0}, many_stat{0}, many_l2_mb{0};   // cluster-per-problem kernel: CTAs per problem (0 auto), threads per CTA (0 auto), 2 = never stationary
+    std::atomic<int64_t> info_many_cluster{0}, info_many_stat{0}, info_many_clusters{0}, info_many_threads{0};   // plan of its last launch
+    std::atomic<int64_t> info_l2_pingpong{0}, info_l2_resident_mb{0}, info_l2_dynamic{0};   // L2 plan of the last register-streaming launch (read-only use)
+    std::atomic<int64_t> l2_bytes{0};              // L2 size the plan is made for: 0 = the device's cudaDevAttrL2CacheSize, other = pretend it is this many bytes (tests)
+    std::atomic<int64_t> info_l2_bytes{0};         // the L2 size the last plan was made for
+    std::atomic<int64_t> info_algo{0};             // kernel the last mp_recover call used (1, 2 or 3)
+    std::atomic<int64_t> info_tc_clusters{0}, info_tc_at{0}, info_tc_stages{0};   // plan of the last batched tensor-core launch (read-only use)
 };
 Options& options();
 void count_launch(int n = 1);
 
 // ---- device info (cached per device) ---------------------------------------------------------------------
 struct DeviceInfo {
-    int device = -1, sm_count = 0, smem_optin = 0, coop = 0;
+    int device = -1, sm_count = 0, smem_optin = 0, coop = 0, l2_bytes = 0;
 };
 mp_status device_info(DeviceInfo* out);
+// The megabyte figures of the L2 plan below were measured on a B200 whose cudaDevAttrL2CacheSize is 132 644 864 bytes (126.5 MiB);
+// on a device (or MIG slice, or carve-out) with another L2 size they are scaled by l2_scale() = that size / 132 644 864, i.e. they
+// are fractions of the L2: reversed order above 0.68 L2, 0.51 L2 pinned above 0.83 L2 (same-order stream), 0.66 L2 pinned above
+// 1.06 L2 (reversed order).  Knob "l2_bytes" overrides the attribute (tests); "info_l2_bytes" reports the size used.
+constexpr double kL2TunedBytes = 132644864.0;
+double l2_scale();
 
 // ---- workspace layout --------------------------------------------------------------------------------------
 // [ctrl: 256 B][x64: B*M doubles][r64: B*Nr doubles][r32: B*Nr floats][keys: B u64, padded][flags ...]
@@ -68,8 +80,9 @@ static inline int round_up(int v, int m) { return (v + m - 1) / m * m; }
 static inline int l2_resident_groups(double dict_bytes, int grid, double group_bytes, double auto_mb = 68.0, double auto_min_mb = 110.0)
 {
     const int64_t knob = options().l2_resident_mb;
-    const double target = knob == 0 ? 1e6 * auto_mb : knob == 1 ? 0.0 : 1e6 * (double)knob;
-    if (!(target > 0.0) || grid < 1 || !(dict_bytes > (knob == 0 ? 1e6 * auto_min_mb : target))) return 0;
+    const double sc = l2_scale();
+    const double target = knob == 0 ? 1e6 * auto_mb * sc : knob == 1 ? 0.0 : 1e6 * (double)knob;
+    if (!(target > 0.0) || grid < 1 || !(dict_bytes > (knob == 0 ? 1e6 * auto_min_mb * sc : target))) return 0;
     return (int)(target / grid / group_bytes);
 }
 
@@ -84,9 +97,10 @@ struct L2Plan { int pingpong, resident_groups, pin_margin; };
 static inline L2Plan l2_plan(double dict_bytes, int grid, double group_bytes, int groups_per_cta, bool can_pingpong)
 {
     L2Plan l;
-    l.pingpong = can_pingpong && (options().pingpong == 2 || (options().pingpong == 0 && dict_bytes > 90e6));
+    l.pingpong = can_pingpong && (options().pingpong == 2 || (options().pingpong == 0 && dict_bytes > 90e6 * l2_scale()));
     l.resident_groups = l.pingpong ? l2_resident_groups(dict_bytes, grid, group_bytes, 88.0, 140.0) : l2_resident_groups(dict_bytes, grid, group_bytes);
-    const int64_t pct = options().pin_margin_pct == 0 ? 10 : options().pin_margin_pct >= 100 ? 0 : options().pin_margin_pct;
+    const int64_t knob_pct = options().pin_margin_pct;
+    const int64_t pct = knob_pct == 0 ? 10 : knob_pct >= 100 ? 0 : knob_pct;
     int e = l.pingpong ? (int)(pct * groups_per_cta / 100) : 0;
     if (groups_per_cta - 2 * e < l.resident_groups + 1) e = (groups_per_cta - l.resident_groups - 1) / 2;
     l.pin_margin = e > 0 ? e : 0;

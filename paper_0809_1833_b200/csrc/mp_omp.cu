@@ -254,7 +254,8 @@ MP_API mp_status mp_recover_omp(const float* psi_t, int N, int M, int64_t ld,
     count_launch();
     int blocks = (M + 7) / 8;
     if (blocks > di.sm_count * 8) blocks = di.sm_count * 8;
-    const int64_t chunk = options().chunk > 0 ? options().chunk : 64;
+    const int64_t chunk_knob = options().chunk;
+    const int64_t chunk = chunk_knob > 0 ? chunk_knob : 64;
     int done_iters = 0;
     while (done_iters < T) {
         const int n = (int)((T - done_iters) < chunk ? (T - done_iters) : chunk);

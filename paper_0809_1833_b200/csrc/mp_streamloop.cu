@@ -162,7 +162,8 @@ mp_status launch_recover_streamloop(const RecoverArgs& a, const Workspace& ws, c
     MP_CUDA(cudaGetLastError());
     int blocks = (a.M + 7) / 8;
     if (blocks > di.sm_count * 8) blocks = di.sm_count * 8;
-    const int64_t chunk = options().chunk > 0 ? options().chunk : 64;
+    const int64_t chunk_knob = options().chunk;
+    const int64_t chunk = chunk_knob > 0 ? chunk_knob : 64;
     int done_iters = 0;
     while (done_iters < a.max_iter) {
         const int n = (int)((a.max_iter - done_iters) < chunk ? (a.max_iter - done_iters) : chunk);

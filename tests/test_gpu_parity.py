@@ -513,6 +513,71 @@ def test_l2_residency_hints_do_not_change_results(mp, N, M, K):
         assert np.array_equal(a, b)
 
 
+def test_l2_plan_scales_with_the_l2_size(mp):
+    """The plan's thresholds are fractions of cudaDevAttrL2CacheSize (mp_internal.h l2_scale): with the attribute overridden to a
+    quarter of this device's L2 through the knob "l2_bytes", a 64 MiB dictionary -- which the real L2 simply holds -- gets what a
+    256 MiB one gets by default (reversed order, a quarter of 88 MB pinned), and the outputs are still the same bits."""
+    N, M = 2048, 8192
+    g = torch.Generator(device="cuda"); g.manual_seed(77)
+    psi = torch.randn(M, N, device="cuda", generator=g); mp.mp_normalize_columns(psi)
+    y = torch.randn(N, device="cuda", generator=g)
+    mp.mp_set_int("algo", 3)
+    try:
+        a = mp.mp_recover(psi, y, 0.0, 24, trace=True); torch.cuda.synchronize()
+        real = mp.mp_get_int("info_l2_bytes")
+        assert real == torch.cuda.get_device_properties(0).L2_cache_size
+        assert mp.mp_get_int("info_l2_pingpong") == 0 and mp.mp_get_int("info_l2_resident_mb") == 0
+        mp.mp_set_int("l2_bytes", real // 4)
+        b = mp.mp_recover(psi, y, 0.0, 24, trace=True); torch.cuda.synchronize()
+        assert mp.mp_get_int("info_l2_bytes") == real // 4 and mp.mp_get_int("info_l2_pingpong") == 1
+        want = 88.0 * (real / 132644864.0) / 4
+        assert abs(mp.mp_get_int("info_l2_resident_mb") - want) <= 3, (mp.mp_get_int("info_l2_resident_mb"), want)
+    finally:
+        mp.mp_set_int("l2_bytes", 0); mp.mp_set_int("algo", 0)
+    assert torch.equal(a.x, b.x) and torch.equal(a.r, b.r) and torch.equal(a.idx_trace, b.idx_trace) and torch.equal(a.c_trace, b.c_trace)
+
+
+def test_two_host_threads_solve_at_once_with_the_same_bits(mp):
+    """include/mp_b200.h: "with the knobs left alone, solves may be issued from several host threads".  Two threads, each with its
+    own stream, outputs and workspace, solve their own cfg1-size signal 40 times while the other does the same (every launch
+    reads the knobs and records its plan in the process-wide info_* fields, which are atomics); every result must be the bits
+    of the same solve done alone."""
+    import threading
+    pb = problems.make_problem(problems.custom_config(256, 1024, 16, eps=1e-5, max_iter=128, B=2), seed=3)
+    psi_d = dev(pb.psi32)
+    ys = [dev(pb.Y[b]) for b in range(2)]
+    alone = [mp.mp_recover(psi_d, ys[b], pb.cfg.eps, pb.cfg.max_iter, trace=True) for b in range(2)]
+    torch.cuda.synchronize()
+    assert all(int(a.n_iter.item()) > 0 for a in alone)
+    errors = []
+
+    def worker(b):
+        try:
+            torch.cuda.set_device(0)
+            s = torch.cuda.Stream()
+            with torch.cuda.stream(s):
+                ws = torch.empty(mp.mp_workspace_bytes(256, 1024, 1) + 256, dtype=torch.uint8, device="cuda")
+                for _ in range(40):
+                    got = mp.mp_recover(psi_d, ys[b], pb.cfg.eps, pb.cfg.max_iter, trace=True, workspace=ws, stream=s)
+                    s.synchronize()
+                    t = int(alone[b].n_iter.item())
+                    ok = (int(got.n_iter.item()) == t and torch.equal(got.x, alone[b].x) and torch.equal(got.r, alone[b].r)
+                          and torch.equal(got.idx_trace[:t], alone[b].idx_trace[:t]) and torch.equal(got.c_trace[:t], alone[b].c_trace[:t]))
+                    if not ok:
+                        errors.append(f"thread {b}: result differs from the solve done alone")
+                        return
+        except Exception as e:                                   # surfaced in the main thread below
+            errors.append(f"thread {b}: {e!r}")
+
+    threads = [threading.Thread(target=worker, args=(b,)) for b in range(2)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join(timeout=120)
+    assert not any(t.is_alive() for t in threads), "a solver thread hangs"
+    assert not errors, errors
+
+
 def test_info_batched_algo_reports_the_path_taken(mp):
     """Auto dispatch may leave the tensor-core kernel (tiny dictionary, refused cooperative launch) and still return MP_OK:
     "info_batched_algo" is how a caller sees which kernel served the last batched call (1 lock-step, 2 sequential, 3 clusters)."""
