@@ -60,6 +60,27 @@ def load_tf32_peak():
     return 1400.0 * ratio, "fallback (B200_PROFILING.md 1.4 PFLOP/s sustained bf16) x 1.1/2.25"
 
 
+K1_SOURCES = ["paper_0809_1833_b200/csrc/mp_persistent_ldg.cu", "paper_0809_1833_b200/csrc/mp_common.cuh", "paper_0809_1833_b200/csrc/mp_internal.h"]
+
+
+def capture_is_stale(capture_commit: str):
+    """A capture of the dominant kernel is only quoted if no later commit touched the kernel's sources: the last commit that did must be
+    the capture's commit or one of its ancestors.  Returns a reason string when stale, "" when fine or when this cannot be told (no .git
+    on the bench box, git missing)."""
+    if not capture_commit or not os.path.isdir(os.path.join(ROOT, ".git")):
+        return ""
+    try:
+        last = subprocess.run(["git", "-C", ROOT, "log", "-1", "--format=%H", "--"] + K1_SOURCES, capture_output=True, text=True, timeout=20)
+        if last.returncode or not last.stdout.strip():
+            return ""
+        anc = subprocess.run(["git", "-C", ROOT, "merge-base", "--is-ancestor", last.stdout.strip(), capture_commit], capture_output=True, timeout=20)
+    except Exception:
+        return ""
+    if anc.returncode == 0:
+        return ""
+    return "captured at %s, but %s touched the kernel's sources later: re-capture" % (capture_commit, last.stdout.strip()[:7])
+
+
 def ncu_traffic(kernel_name: str):
     """DRAM bytes per MP iteration of the dominant kernel -- a CONSTANT read from the committed ncu summary
     profiles/dominant_kernel_traffic.txt (dram__bytes_read.sum + dram__bytes_write.sum of one `ncu --set full` capture, divided
@@ -77,6 +98,9 @@ def ncu_traffic(kernel_name: str):
     if kv.get("kernel", "") not in kernel_name:
         raise SystemExit("profiles/dominant_kernel_traffic.txt is a capture of '%s' but this run launched '%s': re-capture it"
                          % (kv.get("kernel"), kernel_name))
+    stale = capture_is_stale(kv.get("commit", ""))
+    if stale:
+        return None, None, "profiles/dominant_kernel_traffic.txt not used: " + stale
     prov = ("constant from profiles/dominant_kernel_traffic.txt (ncu --set full, %s, commit %s), multiplied by this run's iterations"
             % (kv.get("capture", "?"), kv.get("commit", "?")))
     return float(kv["dram_bytes_per_iteration"].split()[0]), float(kv["dram_bytes_per_iteration_no_hints"].split()[0]), prov
@@ -295,6 +319,14 @@ def probe_read_gbs(torch, mp, dev, nbytes, passes, reps=3):
             "source": "mp_probe_read (read-only 128-bit streaming loop of the single-signal kernel, one CTA per SM), CUDA events, best of %d, this run" % reps}
 
 
+def l2_plan_of(mp):
+    """The L2 plan of the last register-streaming launch, as the library reports it."""
+    return {"reversed_order_on_odd_iterations": bool(mp.mp_get_int("info_l2_pingpong")),
+            "pinned_mb": int(mp.mp_get_int("info_l2_resident_mb")),
+            "items_drawn_from_counter": bool(mp.mp_get_int("info_l2_dynamic")),
+            "l2_bytes": int(mp.mp_get_int("info_l2_bytes"))}   # cudaDevAttrL2CacheSize: the plan's thresholds are fractions of it
+
+
 L2_RESIDENT_MAX_BYTES = 100e6      # dictionaries up to here are served by the 126 MB L2 after the first iteration (DESIGN.md section 5)
 
 
@@ -406,14 +438,11 @@ def main():
     if args.config == "cfg3" and not args.knob and args.max_iter is None and mp.mp_get_int("info_algo") == 3:
         per_it, per_it_off, tsrc = ncu_traffic(mp_kernel_name(mp, False))
     l2p = None
-    if B == 1 and world == 1 and 4.0 * N * M <= L2_RESIDENT_MAX_BYTES:          # cache-resident config: roofline = the L2 read rate at this size
-        l2p = probe_read_gbs(torch, mp, dev, 4.0 * N * M, passes=int(max(50, min(4000, 2.5e10 / (4.0 * N * M)))))
+    if B == 1 and world == 1 and 4.0 * N * M <= L2_RESIDENT_MAX_BYTES:          # cache-resident config: roofline = the L2 read rate (probe over 64 MiB)
+        l2p = probe_read_gbs(torch, mp, dev, 64 << 20, passes=400)
     roofline = roofline_of(mp, cfg, m, per_it, tsrc, l2_probe=l2p)
     if mp.mp_get_int("info_algo") == 3:
-        roofline["l2_plan"] = {"reversed_order_on_odd_iterations": bool(mp.mp_get_int("info_l2_pingpong")),
-                               "pinned_mb": int(mp.mp_get_int("info_l2_resident_mb")),
-                               "items_drawn_from_counter": bool(mp.mp_get_int("info_l2_dynamic")),
-                               "l2_bytes": int(mp.mp_get_int("info_l2_bytes"))}   # cudaDevAttrL2CacheSize: the plan's thresholds are fractions of it
+        roofline["l2_plan"] = l2_plan_of(mp)
     if per_it and "dram_frac" in roofline:
         # frac can exceed 1: ~88 MB of the dictionary are pinned in L2 (L2::evict_last loads) and odd iterations visit the rows in
         # reverse order, so that the rows read last are read first again: the kernel moves fewer HBM bytes per iteration than 4NM.
@@ -459,10 +488,14 @@ def main():
         del wl
         torch.cuda.empty_cache()
         extra = {}
+        # the L2 read rate of this box, once, for every cache-resident leg: the probe over 64 MiB (cfg2's size; north_star: "L2 bandwidth
+        # when Psi fits in L2").  Smaller buffers would under-fill the probe's own grid (8 KiB items, 148 x 16 warps), not the L2.
+        l2p64 = probe_read_gbs(torch, mp, dev, 64 << 20, passes=400)
+        roofline["read_ceiling_l2"] = l2p64
         # the whole size sweep of BASELINE.json configs[3] (4 MiB ... 1 GiB, across the L2-to-HBM transition), cfg1, cfg2 and cfg5
         for name in ("cfg1", "cfg2", "cfg4_2048", "cfg4_4096", "cfg4_8192", "cfg4_16384", "cfg4_32768", "cfg5"):
             small = name in ("cfg1", "cfg4_2048", "cfg4_4096", "cfg4_16384")
-            extra[name] = extra_leg(torch, mp, synth.config(name), local, dev, steps=3 if small else 5)
+            extra[name] = extra_leg(torch, mp, synth.config(name), local, dev, steps=3 if small else 5, l2_probe=l2p64)
 
     if rank == 0:
         print(json.dumps({
@@ -476,17 +509,15 @@ def main():
         dist.destroy_process_group()
 
 
-def extra_leg(torch, mp, cfg, local, dev, steps=5, warmup=3):
+def extra_leg(torch, mp, cfg, local, dev, steps=5, warmup=3, l2_probe=None):
     """One of the other regimes (cfg1, cfg2, the cfg4 sizes: L2-resident up to 64 MiB, 1 GiB from HBM; cfg5: batched tensor-core),
     same protocol as the headline: W warm-ups, K timed steps, CUDA events, nvidia-smi clocks during its own timed region (one retry
-    if that region saw a slowdown flag).  L2-resident sizes are stated against the L2 read rate the probe gives at their own size."""
+    if that region saw a slowdown flag).  L2-resident sizes are stated against the L2 read rate of the probe (roofline.read_ceiling_l2)."""
     wl = Workload(torch, mp, cfg, 1, dev)
     m = wl.timed(steps, warmup, local)
     algo = int(mp.mp_get_int("info_algo")) if cfg.B == 1 else None
-    probe = None
-    if cfg.B == 1 and 4.0 * cfg.N * cfg.M <= L2_RESIDENT_MAX_BYTES:
-        nbytes = 4.0 * cfg.N * cfg.M
-        probe = probe_read_gbs(torch, mp, dev, nbytes, passes=int(max(50, min(4000, 2.5e10 / nbytes))))
+    plan = l2_plan_of(mp) if algo == 3 else None
+    probe = l2_probe if cfg.B == 1 and 4.0 * cfg.N * cfg.M <= L2_RESIDENT_MAX_BYTES else None
     rl = roofline_of(mp, cfg, m, l2_probe=probe)
     out = {"workload": workload_name(cfg), "bound": rl["bound"], "frac": rl["frac"], "achieved": rl["achieved"], "peak": rl["peak"],
            "unit": rl["unit"], "peak_source": rl["peak_source"], "kernel": rl["kernel"], "iterations_per_step": m["its_per_step"],
@@ -495,6 +526,12 @@ def extra_leg(torch, mp, cfg, local, dev, steps=5, warmup=3):
     for k in ("regime", "frac_vs_hbm_peak", "l2_probe"):
         if k in rl:
             out[k] = rl[k]
+    if plan is not None:
+        out["l2_plan"] = plan
+    if rl["bound"] == "hbm" and rl["frac"] > 1.0:
+        out["note"] = ("frac counts the algorithmic 4NM bytes per iteration against the HBM copy peak; it exceeds 1 because part of the dictionary "
+                       "is served by L2 every iteration (l2_plan: pinned rows and/or reversed order on odd iterations), as in the headline "
+                       "(roofline.note, roofline.dram_frac, roofline.no_hint); a read-only stream alone reaches roofline.read_ceiling_hbm")
     if algo is not None:
         out["algo"] = algo
         if algo == 4:

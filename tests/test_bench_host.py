@@ -104,3 +104,22 @@ def test_grading_drift_caps_hold_for_a_run_within_g3_and_catch_one_outside():
                              np.array(idx, np.int32), np.array(c, np.float32), ref=ref, nthreads=1)
     assert g.max_c_err <= grading.C_TOL and g.g1_allowance <= grading.G1_ALLOWANCE_CEILING
     assert grading.G1_ALLOWANCE_MAX_USES >= 33 and grading.N_ITER_DRIFT_MAX_USES >= 1      # the full GPU session's counts fit
+
+
+def test_traffic_capture_is_not_older_than_the_kernel_sources():
+    """profiles/dominant_kernel_traffic.txt (the ncu DRAM traffic bench.py multiplies into roofline.traffic) names the commit it was
+    captured at; no later commit may have touched the dominant kernel's sources.  Needs the git history (skipped without it)."""
+    import subprocess
+    import bench
+    if not os.path.isdir(os.path.join(bench.ROOT, ".git")):
+        pytest.skip("no git history here")
+    kv = {}
+    for line in open(os.path.join(bench.ROOT, "profiles", "dominant_kernel_traffic.txt")):
+        if "=" in line and not line.lstrip().startswith("#"):
+            k, _, v = line.partition("=")
+            kv[k.strip()] = v.split("#")[0].strip()
+    have = subprocess.run(["git", "-C", bench.ROOT, "cat-file", "-e", kv["commit"] + "^{commit}"], capture_output=True)
+    assert have.returncode == 0, "the capture's commit is not in this history"
+    assert bench.capture_is_stale(kv["commit"]) == ""
+    first = subprocess.run(["git", "-C", bench.ROOT, "rev-list", "--max-parents=0", "HEAD"], capture_output=True, text=True).stdout.split()[0]
+    assert "re-capture" in bench.capture_is_stale(first)          # the check does fire for a capture that predates the kernel
