@@ -179,3 +179,14 @@ def test_concurrent_builds_are_serialised_and_the_waiter_does_not_rebuild(monkey
     for t in threads:
         t.join()
     assert state["built"] == 2 and not state["overlap"]
+
+
+def test_probe_read_argument_errors_without_gpu():
+    """mp_probe_read validates on the host: null / misaligned buffer, passes < 1."""
+    from paper_0809_1833_b200.binding import lib
+    ok = C.c_void_p(4096)
+    n = C.c_ulonglong(0)
+    assert lib.mp_probe_read(None, 1 << 24, 1, ok, C.byref(n), None) == 1
+    assert lib.mp_probe_read(ok, 1 << 24, 1, None, C.byref(n), None) == 1
+    assert lib.mp_probe_read(C.c_void_p(4100), 1 << 24, 1, ok, C.byref(n), None) == 1
+    assert lib.mp_probe_read(ok, 1 << 24, 0, ok, C.byref(n), None) == 1

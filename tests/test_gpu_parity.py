@@ -578,6 +578,30 @@ def test_two_host_threads_solve_at_once_with_the_same_bits(mp):
     assert not errors, errors
 
 
+def test_probe_read_reads_what_it_says_and_sums_what_it_read(mp):
+    """mp_probe_read (the read-only ceiling bench.py quotes): the byte count it returns is k x 8 KiB x SMs x passes, a buffer below
+    8 KiB per SM is refused, and the value left in `sink` is the weighted sum of exactly the floats it claims to have read (so the
+    loads are real): with all-ones input each float4 contributes 1.0001 + 0.9999 + 1.0002 + 0.9998 = 4."""
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    unit = sms * 8192
+    buf = torch.ones((3 * unit + 5000) // 4, dtype=torch.float32, device="cuda")
+    sink = torch.zeros(1, dtype=torch.float32, device="cuda")
+    read = mp.mp_probe_read(buf, 2, sink=sink)
+    torch.cuda.synchronize()
+    assert read == 3 * unit * 2
+    assert abs(float(sink.item()) - read / 4.0) <= 2e-3 * read / 4.0          # fp32 accumulation of ~1.8 M ones per warp, summed by atomics
+    with pytest.raises(mp.MPError) as e:
+        mp.mp_probe_read(torch.ones(unit // 4 - 4, dtype=torch.float32, device="cuda"), 1, sink=sink)
+    assert e.value.status == mp.MP_ERR_INVALID_ARG
+    # and it is a bandwidth probe: a 64 MiB buffer read 50 times moves well above the HBM rate (it is served by L2)
+    big = torch.ones((64 << 20) // 4, dtype=torch.float32, device="cuda")
+    mp.mp_probe_read(big, 10, sink=sink); torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(); n = mp.mp_probe_read(big, 50, sink=sink); e1.record(); torch.cuda.synchronize()
+    gbs = n / (e0.elapsed_time(e1) * 1e-3) / 1e9
+    assert gbs > 9000, f"L2-resident probe reads only {gbs:.0f} GB/s"
+
+
 def test_info_batched_algo_reports_the_path_taken(mp):
     """Auto dispatch may leave the tensor-core kernel (tiny dictionary, refused cooperative launch) and still return MP_OK:
     "info_batched_algo" is how a caller sees which kernel served the last batched call (1 lock-step, 2 sequential, 3 clusters)."""
