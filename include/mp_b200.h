@@ -248,9 +248,11 @@ MP_API mp_status mp_recover_many(const float* psi_t, int N, int M, int64_t ld, i
 MP_API const char* mp_last_error(void);
 
 /* Tuning / diagnostic knobs (process-wide, not part of the method).  Unknown name -> MP_ERR_INVALID_ARG.
- * NOT thread-safe: the knobs are plain process-wide variables that every solve reads when it is called.  Set them before
- * solves are issued and do not change them while another host thread is inside a library call; with the knobs left alone,
- * solves may be issued from several host threads (each call keeps its state in its own arguments and workspace).
+ * The knobs and the info_* read-outs are process-wide atomics: setting or reading one never races with a solve on another host
+ * thread, and with the knobs left alone solves may be issued from several host threads at once (each call keeps its state in its
+ * own arguments and workspace; mp_recover_noalloc is the exception, see there).  What stays process-wide is their MEANING: a knob
+ * changed while another thread is inside a library call may or may not apply to that call, and an info_* value is the plan of
+ * whichever launch recorded it last.  Set knobs before the solves they are meant for.
  *   "algo"          0 = auto (default: 4 if one cluster can hold the dictionary in shared memory -- 4NM <= ~3.4 MB, N <= 2048 --
  *                   else 3 if it fits, else 1, else 2), 4 = the cluster kernel of mp_recover_many with P = 1 (N <= 2048),
  *                   1 = persistent cooperative kernel fed by TMA bulk
