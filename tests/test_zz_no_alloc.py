@@ -109,3 +109,47 @@ def test_two_calls_in_a_row_match_the_workspace_path():
             graded = True
     assert graded
     assert mp.mp_launch_count() - launches_before == 4 * len(SHAPES)             # every call above launched its kernel
+
+
+@pytest.mark.gpu
+def test_calls_ordered_on_a_side_stream_do_not_disturb_each_other():
+    """The built-in array is shared by every call on the device, so what keeps calls apart is their order on the GPU.  Here a
+    side stream carries: a no-alloc solve, a workspace solve of another signal, and a no-alloc solve of a third -- enqueued
+    without a host synchronisation in between.  Stream order is all the entry point asks for: each result must be the bits of
+    the same solve done on its own."""
+    import torch
+    import paper_0809_1833_b200 as mp
+
+    N, M, K = 250, 1200, 8
+    T = 3 * K + 2
+    pb = problems.make_problem(problems.custom_config(N, M, K, eps=1e-5, max_iter=T, B=3), seed=41)
+    ld = (N + 3) // 4 * 4
+    buf = torch.zeros((M, ld), dtype=torch.float32, device="cuda")
+    buf[:, :N] = torch.from_numpy(pb.psi32).cuda()
+    psi_d = buf[:, :N]
+    ys = [torch.from_numpy(np.ascontiguousarray(pb.Y[b])).cuda() for b in range(3)]
+    want = [_workspace_path(mp, torch, psi_d, ys[b], pb.cfg.eps, T) for b in range(3)]
+
+    def outputs():
+        return dict(x=torch.empty(M, device="cuda"), r=torch.empty(N, device="cuda"),
+                    n_iter=torch.empty(1, dtype=torch.int32, device="cuda"),
+                    idx_trace=torch.empty(T, dtype=torch.int32, device="cuda"), c_trace=torch.empty(T, device="cuda"))
+
+    outs = [outputs() for _ in range(3)]
+    ws = torch.empty(mp.mp_workspace_bytes(N, M, 1) + 256, dtype=torch.uint8, device="cuda")
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream()
+    mp.mp_set_int("algo", 3)
+    try:
+        mp.mp_recover_noalloc(psi_d, ys[0], pb.cfg.eps, T, stream=side, **outs[0])
+        mp.mp_recover(psi_d, ys[1], pb.cfg.eps, T, workspace=ws, stream=side, **outs[1])
+        mp.mp_recover_noalloc(psi_d, ys[2], pb.cfg.eps, T, stream=side, **outs[2])
+    finally:
+        mp.mp_set_int("algo", 0)
+    side.synchronize()
+    for b in range(3):
+        x, r, t, idx, c = want[b]
+        o = outs[b]
+        assert int(o["n_iter"].item()) == t, b
+        assert np.array_equal(o["idx_trace"].cpu().numpy()[:t], idx) and np.array_equal(o["c_trace"].cpu().numpy()[:t], c), b
+        assert np.array_equal(o["x"].cpu().numpy(), x) and np.array_equal(o["r"].cpu().numpy(), r), b
