@@ -12,7 +12,9 @@ What is checked here:
     finds the array as the first one left it -- give exactly what mp_recover gives on the same inputs with a caller-made
     workspace and the same kernel (knob "algo" = 3).  It is the same arithmetic in the same order, so the comparison is
     bit for bit, which is also what the repository's other same-kernel comparisons use; one result is graded against the
-    float64 oracle as well.  A large-M call precedes a small-M one so that left-over coefficients would show.
+    float64 oracle as well.  A large-M call precedes a small-M one so that left-over coefficients would show;
+  * that no-alloc calls enqueued on a side stream either side of an ordinary workspace solve, with no host synchronisation in
+    between, each still give the bits of the same solve done alone: order on the GPU is all that keeps calls apart.
 
 This file is named to be collected last (pytest -x stops at the first failure, and a failure here must not hide the parity
 tests), and it does not depend on what ran before it: it sets the one knob it needs and puts it back.
