@@ -111,8 +111,9 @@ def test_traffic_capture_is_not_older_than_the_kernel_sources():
     captured at; no later commit may have touched the dominant kernel's sources.  Needs the git history (skipped without it)."""
     import subprocess
     import bench
-    if not os.path.isdir(os.path.join(bench.ROOT, ".git")):
-        pytest.skip("no git history here")
+    import shutil
+    if not os.path.isdir(os.path.join(bench.ROOT, ".git")) or shutil.which("git") is None:
+        pytest.skip("no git history (or no git) here")
     kv = {}
     for line in open(os.path.join(bench.ROOT, "profiles", "dominant_kernel_traffic.txt")):
         if "=" in line and not line.lstrip().startswith("#"):
