@@ -76,7 +76,7 @@ def capture_is_stale(capture_commit: str):
         anc = subprocess.run(["git", "-C", ROOT, "merge-base", "--is-ancestor", last.stdout.strip(), capture_commit], capture_output=True, timeout=20)
     except Exception:
         return ""
-    if anc.returncode == 0:
+    if anc.returncode != 1:               # 0 = ancestor-or-equal: fine; anything but 1 = git could not tell (unknown commit, shallow history)
         return ""
     return "captured at %s, but %s touched the kernel's sources later: re-capture" % (capture_commit, last.stdout.strip()[:7])
 
